@@ -1,0 +1,194 @@
+"""Seeded synthetic inputs for the prefix-cached prefill path (shared by the oracle and the CUDA path).
+
+This module holds NO arithmetic of the method: no ordering, hashing, block management, RoPE or attention.
+It only draws the synthetic RAG traces of SURVEY.md §8(d) (document pools, retrieval lists, queries) and
+the bf16 Q/K/V activations, and concatenates prompt pieces.  Both `oracle/` and the tests/bench of the CUDA
+path import it; neither imports the other.
+
+The traces stand in for the paper's controlled synthetic bursty corpus (§4 "Workload":
+topical regions, ~200-token passages, top-k 5, adjacent-query overlap) and its sweeps (Table 5 top-k,
+Figure 4 overlap, Table 11 concurrency); the authors' generator and traces are not available.
+
+Q/K/V are *keyed by the document prefix*: the activation chunk for document O[j] of a request is drawn from
+a generator seeded by (config seed, O[0..j]); query chunks by (config seed, request index).  Identical
+document prefix => identical pre-RoPE Q/K/V, different prefix => different values, as in a real
+transformer, so a false cache hit cannot pass the "prefix-cached == full recompute" parity check.
+"""
+from __future__ import annotations
+
+from concurrent.futures import ThreadPoolExecutor
+from dataclasses import dataclass, field
+
+import numpy as np
+
+BLOCK_SIZE = 16  # PAPER.md:39 "the token block size is 16 tokens"
+
+
+@dataclass(frozen=True)
+class Config:
+    name: str
+    seed: int
+    n_docs: int          # pool size (per cluster for mode "zipf")
+    doc_len: int
+    n_req: int
+    k: int               # top-k
+    n_shared: int        # docs shared with the previous request (mode "overlap")
+    q_len: int           # query tokens
+    Hq: int
+    Hkv: int
+    D: int
+    NB: int              # KV pool blocks
+    H: int               # recency window (floor(NB / ceil(n/16)))
+    theta: float
+    mode: str = "overlap"    # "overlap" | "zipf"
+    n_clusters: int = 1
+    zipf_s: float = 1.1
+    admission: str = "sequential"   # "sequential" | "waves"
+
+    @property
+    def n(self) -> int:
+        return self.k * self.doc_len + self.q_len
+
+    @property
+    def blocks_per_req(self) -> int:
+        return -(-self.n // BLOCK_SIZE)
+
+    @property
+    def width(self) -> int:
+        """elements per token of the packed [q | k | v] activation row."""
+        return (self.Hq + 2 * self.Hkv) * self.D
+
+
+def n_shared_for(overlap_pct: int, k: int) -> int:
+    """n_shared = floor(overlap*k + 0.5)."""
+    return int(np.floor(overlap_pct / 100.0 * k + 0.5))
+
+
+CONFIGS = {
+    # BASELINE.json configs[0..4]
+    1: Config("cfg1-tiny", 0, 10, 64, 4, 3, 2, 32, 2, 1, 64, 64, 4, 1e4),
+    2: Config("cfg2-llama3-8b", 0, 200, 256, 64, 5, 3, 48, 32, 8, 128, 8192, 98, 5e5),
+    4: Config("cfg4-qwen2.5-7b-concurrent", 0, 50, 512, 256, 10, 0, 64, 28, 4, 128, 32768, 101, 1e6,
+              mode="zipf", n_clusters=8, admission="waves"),
+    5: Config("cfg5-70b-long", 0, 400, 512, 32, 20, 10, 64, 64, 8, 128, 16384, 25, 5e5, admission="waves"),
+}
+
+
+def config3(k: int, overlap_pct: int, n_req: int = 128) -> Config:
+    """Overlap/top-k sweep cell at the 8B shapes (BASELINE.json configs[2]); inherits cfg 2."""
+    n = k * 256 + 48
+    nb = 8192
+    return Config(f"cfg3-k{k}-ov{overlap_pct}", 1000 * k + overlap_pct, 200, 256, n_req, k,
+                  n_shared_for(overlap_pct, k), 48, 32, 8, 128, nb, nb // (-(-n // BLOCK_SIZE)), 5e5)
+
+
+@dataclass
+class Trace:
+    cfg: Config
+    doc_tokens: np.ndarray              # int32 [total_docs, doc_len]
+    retrieval: list                     # n_req lists of int64 doc ids, in retrieval rank
+    query_tokens: np.ndarray            # int32 [n_req, q_len]
+    _chunks: dict = field(default_factory=dict, repr=False)
+
+
+def make_trace(cfg: Config) -> Trace:
+    """Everything derived in a fixed order from one PCG64 generator seeded with cfg.seed."""
+    rng = np.random.default_rng(cfg.seed)
+    total_docs = cfg.n_docs * cfg.n_clusters
+    doc_tokens = rng.integers(0, 32000, size=(total_docs, cfg.doc_len), dtype=np.int32)
+    retrieval = []
+    if cfg.mode == "overlap":
+        prev = None
+        for _ in range(cfg.n_req):
+            if prev is None:
+                docs = rng.choice(total_docs, size=cfg.k, replace=False)
+            else:
+                shared = rng.choice(prev, size=cfg.n_shared, replace=False)
+                rest = np.setdiff1d(np.arange(total_docs), prev)
+                fresh = rng.choice(rest, size=cfg.k - cfg.n_shared, replace=False)
+                docs = np.concatenate([shared, fresh])
+                rng.shuffle(docs)
+            prev = docs.copy()
+            retrieval.append([int(d) for d in docs])
+    elif cfg.mode == "zipf":
+        w = np.arange(1, cfg.n_docs + 1, dtype=np.float64) ** (-cfg.zipf_s)
+        w /= w.sum()
+        for _ in range(cfg.n_req):
+            c = int(rng.integers(0, cfg.n_clusters))
+            docs = rng.choice(cfg.n_docs, size=cfg.k, replace=False, p=w)   # draw order = retrieval order
+            retrieval.append([int(c * cfg.n_docs + d) for d in docs])
+    else:
+        raise ValueError(cfg.mode)
+    query_tokens = rng.integers(0, 32000, size=(cfg.n_req, cfg.q_len), dtype=np.int32)
+    return Trace(cfg, doc_tokens, retrieval, query_tokens)
+
+
+def jaccard(a, b) -> float:
+    """|A∩B|/|A∪B| between two retrieved sets — a trace statistic, not part of the method."""
+    a, b = set(a), set(b)
+    return len(a & b) / len(a | b)
+
+
+def assemble_prompt(trace: Trace, r: int, order) -> np.ndarray:
+    """a3: tokens = doc_tokens[O[0]] ‖ … ‖ doc_tokens[O[k-1]] ‖ query_tokens[r] (north_star: docs then query)."""
+    parts = [trace.doc_tokens[d] for d in order] + [trace.query_tokens[r]]
+    return np.ascontiguousarray(np.concatenate(parts), dtype=np.int32)
+
+
+def f32_to_bf16_bits(x: np.ndarray) -> np.ndarray:
+    """float32 -> bf16 bit pattern (uint16), round-to-nearest-even.  Input conversion only."""
+    u = np.ascontiguousarray(x, dtype=np.float32).view(np.uint32)
+    return ((u + np.uint32(0x7FFF) + ((u >> np.uint32(16)) & np.uint32(1))) >> np.uint32(16)).astype(np.uint16)
+
+
+def bf16_bits_to_f64(b: np.ndarray) -> np.ndarray:
+    """bf16 bit pattern (uint16) -> float64, exact."""
+    return (np.ascontiguousarray(b, dtype=np.uint16).astype(np.uint32) << np.uint32(16)).view(np.float32).astype(np.float64)
+
+
+def _chunk(seed: int, key: tuple, length: int, width: int) -> np.ndarray:
+    g = np.random.Generator(np.random.PCG64(np.random.SeedSequence([seed, *key])))
+    return f32_to_bf16_bits(g.standard_normal((length, width), dtype=np.float32))
+
+
+def qkv_chunk_keys(trace: Trace, r: int, order):
+    """(key, length) of each activation chunk of request r's prompt under `order`."""
+    cfg = trace.cfg
+    keys = [((0, *[int(d) for d in order[: j + 1]]), cfg.doc_len) for j in range(len(order))]
+    keys.append(((1, int(r)), cfg.q_len))
+    return keys
+
+
+def prompt_qkv(trace: Trace, r: int, order, start: int = 0, cache: bool = False) -> np.ndarray:
+    """bf16 bits, uint16 [n - start, (Hq+2Hkv)*D]: packed rows [q heads | k heads | v heads] for prompt
+    positions start..n-1 of request r under `order`.  N(0,1) rounded to bf16 (BASELINE.json configs)."""
+    cfg = trace.cfg
+    out, pos = [], 0
+    for key, length in qkv_chunk_keys(trace, r, order):
+        if pos + length > start:
+            if cache and key in trace._chunks:
+                c = trace._chunks[key]
+            else:
+                c = _chunk(cfg.seed, key, length, cfg.width)
+                if cache:
+                    trace._chunks[key] = c
+            out.append(c[max(0, start - pos):])
+        pos += length
+    return np.concatenate(out, axis=0)
+
+
+def batch_suffix_qkv(trace: Trace, items, threads: int = 8) -> np.ndarray:
+    """items: list of (r, order, n_cached).  Returns the concatenated suffix rows (uint16 [T, width])."""
+    with ThreadPoolExecutor(max_workers=threads) as ex:
+        parts = list(ex.map(lambda it: prompt_qkv(trace, it[0], it[1], it[2]), items))
+    return np.concatenate(parts, axis=0)
+
+
+def split_qkv(cfg: Config, rows: np.ndarray):
+    """packed rows -> (q [T,Hq,D], k [T,Hkv,D], v [T,Hkv,D]) contiguous copies (uint16 bf16 bits)."""
+    T = rows.shape[0]
+    a, b = cfg.Hq * cfg.D, (cfg.Hq + cfg.Hkv) * cfg.D
+    q = np.ascontiguousarray(rows[:, :a]).reshape(T, cfg.Hq, cfg.D)
+    k = np.ascontiguousarray(rows[:, a:b]).reshape(T, cfg.Hkv, cfg.D)
+    v = np.ascontiguousarray(rows[:, b:]).reshape(T, cfg.Hkv, cfg.D)
+    return q, k, v
