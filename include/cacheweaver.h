@@ -1,0 +1,151 @@
+/* cacheweaver.h — C ABI of the B200-native prefix-cached prefill path of CacheWeaver
+ * (arxiv/paper_2606_19667).  Citations are PAPER.md:<line> (+ section / algorithm) and DESIGN.md readings.
+ *
+ * The path:  cw_order -> cw_observe -> cw_lookup -> cw_append_kv -> cw_prefill_attn -> cw_release
+ *
+ * Conventions
+ *   - every function returns int: CW_OK (0) or a negative CW_ERR_*; no exception crosses the ABI.
+ *   - "host" / "device" is stated for every pointer.  The library allocates NO device memory: the caller
+ *     (PyTorch in the binding) owns pools, tables, activations and the stream; `stream` is a cudaStream_t
+ *     passed as void*.  All kernel launches are asynchronous on that stream.
+ *   - out_* arrays are caller-allocated; request handles are library-owned until cw_release.
+ *   - a context is not thread-safe: one context per caller thread.
+ *   - block size is 16 tokens ("the token block size is 16 tokens").
+ */
+#ifndef CACHEWEAVER_H
+#define CACHEWEAVER_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CW_BLOCK_SIZE 16
+
+enum {
+    CW_OK = 0,
+    CW_ERR_INVALID = -1,     /* null pointer, k < 0, duplicate doc id, n <= 0, bad head config, bad sizes   */
+    CW_ERR_NO_SPACE = -2,    /* not enough evictable blocks; library state is unchanged                     */
+    CW_ERR_BAD_HANDLE = -3,  /* unknown / already released request handle                                   */
+    CW_ERR_CUDA = -4         /* CUDA runtime / launch error; text via cw_last_error                         */
+};
+
+typedef struct cw_ctx cw_ctx; /* opaque, created by cw_create, freed by cw_destroy */
+
+typedef struct {
+    int32_t block_size;      /* must be 16                                                    */
+    int32_t num_blocks;      /* NB: blocks in the paged KV pool                                             */
+    int32_t num_q_heads;     /* Hq                                                                          */
+    int32_t num_kv_heads;    /* Hkv, Hq % Hkv == 0 (GQA group g = Hq/Hkv)                                   */
+    int32_t head_dim;        /* D in {64, 128}                                                              */
+    int32_t max_position;    /* rows of the RoPE table = largest prompt length accepted                     */
+    double  rope_theta;      /* RoPE base (reading c4)                                            */
+    int32_t recency_window;  /* H: isCached(node) <=> seq - last_seq < H           */
+    int32_t eager_register;  /* 1: new full blocks enter the prefix index inside cw_lookup; 0: at release    */
+    uint64_t hash_salt;      /* parent hash of block 0 (reading c2)                               */
+    void*   k_pool;          /* device, caller-owned, cw_pool_bytes() bytes, bf16, layout: see cw_pool_offset */
+    void*   v_pool;          /* device, caller-owned, same size/layout                                      */
+    void*   rope_table;      /* device, caller-owned, max_position*(D/2)*2 fp32 {cos,sin}; FILLED by cw_create.
+                                may be NULL together with k_pool/v_pool for a host-only context (no kernels) */
+    int32_t device;          /* CUDA device ordinal (ignored for a host-only context)                       */
+} cw_config;
+
+typedef struct {
+    int64_t requests;        /* successful non-peek lookups                                                 */
+    int64_t hit_blocks;      /* sum of m over those lookups                                                 */
+    int64_t miss_blocks;     /* sum of ceil(n/16) - m                                                       */
+    int64_t evictions;       /* hashed blocks whose index entry was dropped by allocation                   */
+    int64_t trie_nodes;      /* live trie nodes (root excluded)                                             */
+    int64_t order_probes;    /* child probes of the last cw_order call (<= k(k+1)/2)          */
+    int64_t free_blocks;     /* current length of the LRU free list                                         */
+    int64_t seq;             /* number of cw_observe calls so far                                           */
+} cw_stats_t;
+
+/* ---- lifetime ---------------------------------------------------------------------------------------- */
+/* Validates cfg, builds host state (trie, index, LRU list 0..NB-1), and — unless host-only — computes the
+ * RoPE {cos,sin} table in fp64 on the host, rounds to fp32 and copies it to cfg->rope_table (synchronous). */
+int  cw_create(const cw_config* cfg, cw_ctx** out);
+void cw_destroy(cw_ctx* ctx);
+const char* cw_strerror(int code);
+const char* cw_last_error(cw_ctx* ctx);  /* text of the last CW_ERR_CUDA / CW_ERR_INVALID on this context */
+int  cw_stats(cw_ctx* ctx, cw_stats_t* out);
+/* bytes of ONE pool tensor (K or V): NB * Hkv * 16 * D * 2 */
+int64_t cw_pool_bytes(const cw_config* cfg);
+/* element offset (in bf16 elements) inside a pool tensor of element (block, kv_head, token-in-block t, dim d).
+ * The in-block layout is the tcgen05 "canonical 128B-swizzled" tile so one (block, kv head) run of 16*D*2 bytes
+ * is moved by ONE bulk copy and consumed by the MMA without re-layout:
+ *   off = ((block*Hkv + kv_head) * 16*D) + (t/8)*(8*D) + (d/64)*512 + (t%8)*64 + ((((d%64)/8) ^ (t%8))*8) + d%8 */
+int64_t cw_pool_offset(const cw_config* cfg, int32_t block, int32_t kv_head, int32_t t, int32_t d);
+
+/* ---- ordering, host (PAPER.md:57 knowledge tree; Algorithm 1) ------------------------- */
+/* Algorithm 1: doc_ids[k] in retrieval rank (host, distinct) -> out_order[k] (host); *out_pred_prefix_docs =
+ * l(O,T), the depth of the cached trie path followed.  k == 0 is OK (empty order).
+ * Pure: does not modify the tree.  Duplicate ids -> CW_ERR_INVALID (D is a set). */
+int cw_order(cw_ctx* ctx, const int64_t* doc_ids, int32_t k, int64_t* out_order, int32_t* out_pred_prefix_docs);
+/* l(O,T) of a given order without reordering it (retrieval-order arm). */
+int cw_predict(cw_ctx* ctx, const int64_t* order, int32_t k, int32_t* out_prefix_docs);
+/* "After a request finishes, its ordered document sequence is inserted": seq += 1, create the
+ * path, stamp last_seq on every node of it; nodes outside the recency window are pruned lazily. */
+int cw_observe(cw_ctx* ctx, const int64_t* ordered_doc_ids, int32_t k);
+
+/* ---- prefix cache, host (PAPER.md:33 chained block hashes; PAPER.md:129 block eviction) -------------- */
+/* chain[i] = FNV1a64(LE64(chain[i-1]) || 16 x LE32(token)), chain[-1] = hash_salt, i < floor(n/16). */
+int cw_hash_chain(cw_ctx* ctx, const int32_t* tokens, int32_t n, uint64_t* out_chain);
+/* Longest resident prefix + pin + allocate + evict + register (reading c3).
+ *   tokens[n] host.  m = leading chain hashes found in the index, capped at floor((n-1)/16).
+ *   peek_only = 1: only *out_n_cached = 16*m is written; no state change, out_req/out_block_table untouched.
+ *   else: out_block_table[ceil(n/16)] (host) receives the block ids, *out_req the handle, *out_n_cached = 16*m.
+ *   CW_ERR_NO_SPACE leaves every piece of state unchanged. */
+int cw_lookup(cw_ctx* ctx, const int32_t* tokens, int32_t n, int32_t peek_only,
+              int64_t* out_req, int32_t* out_block_table, int32_t* out_n_cached);
+/* Unpin; blocks whose refcount reaches 0 go to the LRU tail in REVERSE block order. */
+int cw_release(cw_ctx* ctx, int64_t req);
+/* Copy the LRU free list head->tail into out[cap] (host); returns its length via *out_len (testing aid). */
+int cw_free_list(cw_ctx* ctx, int32_t* out, int32_t cap, int32_t* out_len);
+
+/* ---- device work (async on `stream`) ----------------------------------------------------------------- */
+/* Batch of B requests; request r owns suffix rows cu_seqlens_q[r]..cu_seqlens_q[r+1]-1 (T rows in total),
+ * row i of request r sits at absolute prompt position n_cached[r] + i.  All d_* pointers are DEVICE int32.
+ * d_block_tables is [B, max_blocks_per_req] row-major.
+ *
+ * cw_append_kv — fused RoPE + KV scatter (kernel 1):  for each suffix token at position p
+ *     q_roped = RoPE(q, p);  pool_K[slot(p)] = RoPE(k, p);  pool_V[slot(p)] = v;
+ *     slot(p) = (block_table[p/16], p%16)          (DESIGN.md c4 split-half RoPE)
+ *   q [T,Hq,D], k,v [T,Hkv,D], q_roped [T,Hq,D]: device bf16, row-major contiguous; q_roped must NOT alias q
+ *   (q is read through the non-coherent path).  Positions >= max_position are invalid.  The pools must have been
+ *   zero-filled once by the caller (stale slots of a partially filled block must hold finite values). */
+int cw_append_kv(cw_ctx* ctx, const void* q, const void* k, const void* v, void* q_roped,
+                 const int32_t* d_cu_seqlens_q, const int32_t* d_n_cached, const int32_t* d_block_tables,
+                 int32_t max_blocks_per_req, int32_t B, int32_t T, void* stream);
+
+/* cw_prefill_attn — varlen paged causal GQA attention of the suffix rows (kernel 2):
+ *     o[row p, head h] = sum_{j<=p} softmax_j(q'_p . k'_j / sqrt(D)) v_j, kv head = h / g, keys j read from the
+ *     pool through the block table (cached prefix j < n_cached and the blocks just written by cw_append_kv).
+ *   h_cu_seqlens_q [B+1], h_n_cached [B]: HOST copies of the same descriptors (used only to build the tile
+ *   schedule on the host; kv_len[r] = n_cached[r] + suffix length).  d_work: DEVICE int32 scratch of
+ *   cw_attn_work_ints(...) ints, caller-owned, filled asynchronously on `stream` by this call.
+ *   q_roped, out [T,Hq,D] device bf16. */
+int64_t cw_attn_work_ints(cw_ctx* ctx, const int32_t* h_cu_seqlens_q, int32_t B);
+int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out,
+                    const int32_t* h_cu_seqlens_q, const int32_t* h_n_cached,
+                    const int32_t* d_cu_seqlens_q, const int32_t* d_n_cached, const int32_t* d_block_tables,
+                    int32_t max_blocks_per_req, int32_t B, int32_t T, int32_t* d_work, void* stream);
+
+/* cw_gather_kv — export: pool -> plain row-major k_out, v_out [n, Hkv, D] bf16 (device) for one block table
+ * (device int32 [ceil(n/16)]).  Used by tests and by callers that want the cached KV in a plain layout. */
+int cw_gather_kv(cw_ctx* ctx, const int32_t* d_block_table, int32_t n, void* k_out, void* v_out, void* stream);
+
+/* cw_prefill_host — the same path with HOST buffers (end-to-end entry point): copies q,k,v and the descriptors
+ * to the caller-owned device workspace `d_ws` (cw_prefill_host_ws_bytes bytes), runs cw_append_kv +
+ * cw_prefill_attn, copies out [T,Hq,D] back to host and synchronises the stream.  Host buffers should be pinned.
+ * h_block_tables is [B, max_blocks_per_req]. */
+int64_t cw_prefill_host_ws_bytes(cw_ctx* ctx, int32_t B, int32_t T, int32_t max_blocks_per_req);
+int cw_prefill_host(cw_ctx* ctx, const void* h_q, const void* h_k, const void* h_v, void* h_out,
+                    const int32_t* h_cu_seqlens_q, const int32_t* h_n_cached, const int32_t* h_block_tables,
+                    int32_t max_blocks_per_req, int32_t B, int32_t T, void* d_ws, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CACHEWEAVER_H */

@@ -1,0 +1,243 @@
+"""ctypes binding of libcacheweaver.so — argument marshalling only; every step of the path runs in the library.
+
+The function names are those of include/cacheweaver.h.  PyTorch is used for device memory and streams.
+There is no fallback: if the library is missing or a kernel is requested without CUDA, this raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libcacheweaver.so")
+
+CW_OK, CW_ERR_INVALID, CW_ERR_NO_SPACE, CW_ERR_BAD_HANDLE, CW_ERR_CUDA = 0, -1, -2, -3, -4
+BLOCK_SIZE = 16
+
+
+class CwConfig(C.Structure):
+    _fields_ = [("block_size", C.c_int32), ("num_blocks", C.c_int32), ("num_q_heads", C.c_int32),
+                ("num_kv_heads", C.c_int32), ("head_dim", C.c_int32), ("max_position", C.c_int32),
+                ("rope_theta", C.c_double), ("recency_window", C.c_int32), ("eager_register", C.c_int32),
+                ("hash_salt", C.c_uint64), ("k_pool", C.c_void_p), ("v_pool", C.c_void_p),
+                ("rope_table", C.c_void_p), ("device", C.c_int32)]
+
+
+class CwStats(C.Structure):
+    _fields_ = [(n, C.c_int64) for n in ("requests", "hit_blocks", "miss_blocks", "evictions", "trie_nodes",
+                                          "order_probes", "free_blocks", "seq")]
+
+
+class CwError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"cacheweaver error {code}: {msg}")
+        self.code = code
+
+
+class NoSpace(CwError):
+    pass
+
+
+_lib = None
+
+
+def load_library(build_if_missing: bool = True):
+    """dlopen libcacheweaver.so (building it in-tree with nvcc if it is missing).  Fails loudly otherwise."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        if not build_if_missing:
+            raise OSError(f"{LIB_PATH} not built; run python -m paper_2606_19667_b200.build")
+        from .build import build
+        build()
+    lib = C.CDLL(LIB_PATH)
+    p, i32, i64, vp = C.POINTER, C.c_int32, C.c_int64, C.c_void_p
+    sig = {
+        "cw_create": (C.c_int, [p(CwConfig), p(vp)]),
+        "cw_destroy": (None, [vp]),
+        "cw_strerror": (C.c_char_p, [C.c_int]),
+        "cw_last_error": (C.c_char_p, [vp]),
+        "cw_stats": (C.c_int, [vp, p(CwStats)]),
+        "cw_pool_bytes": (i64, [p(CwConfig)]),
+        "cw_pool_offset": (i64, [p(CwConfig), i32, i32, i32, i32]),
+        "cw_order": (C.c_int, [vp, p(i64), i32, p(i64), p(i32)]),
+        "cw_predict": (C.c_int, [vp, p(i64), i32, p(i32)]),
+        "cw_observe": (C.c_int, [vp, p(i64), i32]),
+        "cw_hash_chain": (C.c_int, [vp, p(i32), i32, p(C.c_uint64)]),
+        "cw_lookup": (C.c_int, [vp, p(i32), i32, i32, p(i64), p(i32), p(i32)]),
+        "cw_release": (C.c_int, [vp, i64]),
+        "cw_free_list": (C.c_int, [vp, p(i32), i32, p(i32)]),
+        "cw_append_kv": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp]),
+        "cw_attn_work_ints": (i64, [vp, p(i32), i32]),
+        "cw_prefill_attn": (C.c_int, [vp, vp, vp, p(i32), p(i32), vp, vp, vp, i32, i32, i32, vp, vp]),
+        "cw_gather_kv": (C.c_int, [vp, vp, i32, vp, vp, vp]),
+        "cw_prefill_host_ws_bytes": (i64, [vp, i32, i32, i32]),
+        "cw_prefill_host": (C.c_int, [vp, vp, vp, vp, vp, p(i32), p(i32), p(i32), i32, i32, i32, vp, vp]),
+    }
+    for name, (res, args) in sig.items():
+        f = getattr(lib, name)
+        f.restype, f.argtypes = res, args
+    _lib = lib
+    return lib
+
+
+EXPORTS = ["cw_create", "cw_destroy", "cw_strerror", "cw_last_error", "cw_stats", "cw_pool_bytes", "cw_pool_offset",
+           "cw_order", "cw_predict", "cw_observe", "cw_hash_chain", "cw_lookup", "cw_release", "cw_free_list",
+           "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_gather_kv", "cw_prefill_host_ws_bytes",
+           "cw_prefill_host"]
+
+
+def _i32p(a):
+    return a.ctypes.data_as(C.POINTER(C.c_int32))
+
+
+def _i64p(a):
+    return a.ctypes.data_as(C.POINTER(C.c_int64))
+
+
+def _np_i32(x):
+    return np.ascontiguousarray(x, dtype=np.int32)
+
+
+class Context:
+    """One cw_ctx.  device=None -> host-only context (ordering + prefix cache, no kernels, no CUDA needed)."""
+
+    def __init__(self, num_blocks, num_q_heads, num_kv_heads, head_dim, recency_window, rope_theta=10000.0,
+                 max_position=0, eager_register=True, hash_salt=0, device=None):
+        self.lib = load_library()
+        self.device = device
+        self.Hq, self.Hkv, self.D, self.NB = num_q_heads, num_kv_heads, head_dim, num_blocks
+        cfg = CwConfig(BLOCK_SIZE, num_blocks, num_q_heads, num_kv_heads, head_dim, max_position, float(rope_theta),
+                       recency_window, int(bool(eager_register)), hash_salt, None, None, None, 0)
+        self.k_pool = self.v_pool = self.rope_table = None
+        if device is not None:
+            import torch
+            if not torch.cuda.is_available():
+                raise RuntimeError("a device context needs CUDA; there is no CPU fallback")
+            dev = torch.device(device)
+            nbytes = self.lib.cw_pool_bytes(C.byref(cfg))
+            if nbytes < 0:
+                raise CwError(int(nbytes), "bad configuration")
+            # zero-filled once: stale slots of a partially filled block must hold finite values (cacheweaver.h)
+            self.k_pool = torch.zeros(nbytes // 2, dtype=torch.bfloat16, device=dev)
+            self.v_pool = torch.zeros(nbytes // 2, dtype=torch.bfloat16, device=dev)
+            self.rope_table = torch.empty(max_position * head_dim, dtype=torch.float32, device=dev)
+            cfg.k_pool, cfg.v_pool, cfg.rope_table = self.k_pool.data_ptr(), self.v_pool.data_ptr(), self.rope_table.data_ptr()
+            cfg.device = dev.index or 0
+        self.cfg = cfg
+        h = C.c_void_p()
+        rc = self.lib.cw_create(C.byref(cfg), C.byref(h))
+        if rc != CW_OK:
+            raise CwError(rc, self.lib.cw_strerror(rc).decode())
+        self.h = h
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.cw_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc == CW_OK:
+            return
+        msg = self.lib.cw_strerror(rc).decode()
+        if rc in (CW_ERR_CUDA, CW_ERR_INVALID):
+            msg += ": " + self.lib.cw_last_error(self.h).decode()
+        raise (NoSpace if rc == CW_ERR_NO_SPACE else CwError)(rc, msg)
+
+    # ---- ordering ----
+    def cw_order(self, doc_ids):
+        d = np.ascontiguousarray(doc_ids, dtype=np.int64)
+        out = np.empty_like(d)
+        depth = C.c_int32()
+        self._check(self.lib.cw_order(self.h, _i64p(d), len(d), _i64p(out), C.byref(depth)))
+        return out.tolist(), depth.value
+
+    def cw_predict(self, order):
+        d = np.ascontiguousarray(order, dtype=np.int64)
+        depth = C.c_int32()
+        self._check(self.lib.cw_predict(self.h, _i64p(d), len(d), C.byref(depth)))
+        return depth.value
+
+    def cw_observe(self, order):
+        d = np.ascontiguousarray(order, dtype=np.int64)
+        self._check(self.lib.cw_observe(self.h, _i64p(d), len(d)))
+
+    # ---- prefix cache ----
+    def cw_hash_chain(self, tokens):
+        t = _np_i32(tokens)
+        out = np.empty(len(t) // BLOCK_SIZE, dtype=np.uint64)
+        self._check(self.lib.cw_hash_chain(self.h, _i32p(t), len(t), out.ctypes.data_as(C.POINTER(C.c_uint64))))
+        return out
+
+    def cw_lookup(self, tokens, peek_only=False):
+        t = _np_i32(tokens)
+        n = len(t)
+        nc = C.c_int32()
+        if peek_only:
+            self._check(self.lib.cw_lookup(self.h, _i32p(t), n, 1, None, None, C.byref(nc)))
+            return nc.value
+        table = np.empty(-(-n // BLOCK_SIZE), dtype=np.int32)
+        req = C.c_int64()
+        self._check(self.lib.cw_lookup(self.h, _i32p(t), n, 0, C.byref(req), _i32p(table), C.byref(nc)))
+        return req.value, table, nc.value
+
+    def cw_release(self, req):
+        self._check(self.lib.cw_release(self.h, req))
+
+    def cw_free_list(self):
+        out = np.empty(self.NB, dtype=np.int32)
+        n = C.c_int32()
+        self._check(self.lib.cw_free_list(self.h, _i32p(out), self.NB, C.byref(n)))
+        return out[: n.value].tolist()
+
+    def cw_stats(self):
+        s = CwStats()
+        self._check(self.lib.cw_stats(self.h, C.byref(s)))
+        return {n: getattr(s, n) for n, _ in CwStats._fields_}
+
+    def cw_pool_offset(self, block, kv_head, t, d):
+        return self.lib.cw_pool_offset(C.byref(self.cfg), block, kv_head, t, d)
+
+    # ---- device work ----
+    @staticmethod
+    def _stream():
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+
+    def cw_append_kv(self, q, k, v, q_roped, d_cu, d_nc, d_tables, max_blocks, B, T):
+        self._check(self.lib.cw_append_kv(self.h, q.data_ptr(), k.data_ptr(), v.data_ptr(), q_roped.data_ptr(),
+                                          d_cu.data_ptr(), d_nc.data_ptr(), d_tables.data_ptr(), max_blocks, B, T,
+                                          self._stream()))
+
+    def cw_attn_work_ints(self, h_cu):
+        h_cu = _np_i32(h_cu)
+        return int(self.lib.cw_attn_work_ints(self.h, _i32p(h_cu), len(h_cu) - 1))
+
+    def cw_prefill_attn(self, q_roped, out, h_cu, h_nc, d_cu, d_nc, d_tables, max_blocks, B, T, d_work):
+        h_cu, h_nc = _np_i32(h_cu), _np_i32(h_nc)
+        self._check(self.lib.cw_prefill_attn(self.h, q_roped.data_ptr(), out.data_ptr(), _i32p(h_cu), _i32p(h_nc),
+                                             d_cu.data_ptr(), d_nc.data_ptr(), d_tables.data_ptr(), max_blocks, B, T,
+                                             d_work.data_ptr(), self._stream()))
+
+    def cw_gather_kv(self, d_table, n, k_out, v_out):
+        self._check(self.lib.cw_gather_kv(self.h, d_table.data_ptr(), n, k_out.data_ptr(), v_out.data_ptr(),
+                                          self._stream()))
+
+    def cw_prefill_host_ws_bytes(self, B, T, max_blocks):
+        return int(self.lib.cw_prefill_host_ws_bytes(self.h, B, T, max_blocks))
+
+    def cw_prefill_host(self, h_q, h_k, h_v, h_out, h_cu, h_nc, h_tables, max_blocks, B, T, d_ws):
+        """h_q/h_k/h_v/h_out: pinned CPU torch tensors (bf16); descriptors: numpy int32; d_ws: device uint8 tensor."""
+        h_cu, h_nc, h_tables = _np_i32(h_cu), _np_i32(h_nc), _np_i32(h_tables)
+        self._check(self.lib.cw_prefill_host(self.h, h_q.data_ptr(), h_k.data_ptr(), h_v.data_ptr(), h_out.data_ptr(),
+                                             _i32p(h_cu), _i32p(h_nc), _i32p(h_tables), max_blocks, B, T,
+                                             d_ws.data_ptr(), self._stream()))

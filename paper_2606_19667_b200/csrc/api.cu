@@ -1,0 +1,298 @@
+// C ABI of libcacheweaver.so (include/cacheweaver.h): argument checking, error mapping and glue only.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstring>
+#include <new>
+#include <unordered_set>
+
+#include "cw_internal.h"
+
+namespace {
+
+int fail(cw_ctx* ctx, int code, const char* msg) {
+    if (ctx) ctx->last_error = msg;
+    return code;
+}
+int cuda_fail(cw_ctx* ctx, int cuda_err, const char* where) {
+    ctx->last_error = std::string(where) + ": " + cudaGetErrorString((cudaError_t)cuda_err);
+    return CW_ERR_CUDA;
+}
+bool bad_cfg(const cw_config* c) {
+    return !c || c->block_size != CW_BLOCK_SIZE || c->num_blocks <= 0 || c->num_q_heads <= 0 || c->num_kv_heads <= 0 ||
+           c->num_q_heads % c->num_kv_heads != 0 || (c->head_dim != 64 && c->head_dim != 128) || c->recency_window <= 0;
+}
+inline int64_t align256(int64_t x) { return (x + 255) / 256 * 256; }
+
+}  // namespace
+
+extern "C" {
+
+const char* cw_strerror(int code) {
+    switch (code) {
+        case CW_OK: return "ok";
+        case CW_ERR_INVALID: return "invalid argument";
+        case CW_ERR_NO_SPACE: return "not enough evictable KV blocks";
+        case CW_ERR_BAD_HANDLE: return "unknown request handle";
+        case CW_ERR_CUDA: return "CUDA error";
+        default: return "unknown error code";
+    }
+}
+
+const char* cw_last_error(cw_ctx* ctx) { return ctx ? ctx->last_error.c_str() : ""; }
+
+int64_t cw_pool_bytes(const cw_config* c) {
+    if (bad_cfg(c)) return CW_ERR_INVALID;
+    return (int64_t)c->num_blocks * c->num_kv_heads * CW_BLOCK_SIZE * c->head_dim * 2;
+}
+
+int64_t cw_pool_offset(const cw_config* c, int32_t block, int32_t kv_head, int32_t t, int32_t d) {
+    if (bad_cfg(c) || block < 0 || block >= c->num_blocks || kv_head < 0 || kv_head >= c->num_kv_heads || t < 0 ||
+        t >= CW_BLOCK_SIZE || d < 0 || d >= c->head_dim)
+        return CW_ERR_INVALID;
+    const int64_t D = c->head_dim;
+    return ((int64_t)block * c->num_kv_heads + kv_head) * (CW_BLOCK_SIZE * D) + (t / 8) * (8 * D) + (d / 64) * 512 +
+           (t % 8) * 64 + ((((d % 64) / 8) ^ (t % 8)) * 8) + d % 8;
+}
+
+int cw_create(const cw_config* cfg, cw_ctx** out) {
+    if (!out || bad_cfg(cfg)) return CW_ERR_INVALID;
+    const bool host_only = !cfg->k_pool && !cfg->v_pool && !cfg->rope_table;
+    if (!host_only && (!cfg->k_pool || !cfg->v_pool || !cfg->rope_table || cfg->max_position <= 0 || !(cfg->rope_theta > 0)))
+        return CW_ERR_INVALID;
+    cw_ctx* ctx = new (std::nothrow) cw_ctx();
+    if (!ctx) return CW_ERR_INVALID;
+    ctx->cfg = *cfg;
+    ctx->host_only = host_only;
+    ctx->num_sms = 148;
+    ctx->tree = new cw::KnowledgeTree(cfg->recency_window);
+    ctx->blocks = new cw::BlockManager(cfg->num_blocks, cfg->eager_register != 0, cfg->hash_salt);
+    if (!host_only) {
+        cudaError_t e = cudaSetDevice(cfg->device);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, cfg->device);
+        if (e == cudaSuccess) {
+            // RoPE table (DESIGN.md c4): angle = p * theta^(-2i/D) evaluated in fp64, {cos, sin} rounded once to fp32
+            const int half = cfg->head_dim / 2;
+            std::vector<float> tab((size_t)cfg->max_position * half * 2);
+            std::vector<double> inv((size_t)half);
+            for (int i = 0; i < half; ++i) inv[(size_t)i] = std::pow(cfg->rope_theta, -2.0 * i / cfg->head_dim);
+            for (int64_t p = 0; p < cfg->max_position; ++p)
+                for (int i = 0; i < half; ++i) {
+                    const double a = (double)p * inv[(size_t)i];
+                    tab[((size_t)p * half + i) * 2] = (float)std::cos(a);
+                    tab[((size_t)p * half + i) * 2 + 1] = (float)std::sin(a);
+                }
+            e = cudaMemcpy(cfg->rope_table, tab.data(), tab.size() * sizeof(float), cudaMemcpyHostToDevice);
+        }
+        if (e != cudaSuccess) {
+            cw_destroy(ctx);
+            return CW_ERR_CUDA;
+        }
+    }
+    *out = ctx;
+    return CW_OK;
+}
+
+void cw_destroy(cw_ctx* ctx) {
+    if (!ctx) return;
+    delete ctx->tree;
+    delete ctx->blocks;
+    delete ctx;
+}
+
+int cw_stats(cw_ctx* ctx, cw_stats_t* o) {
+    if (!ctx || !o) return CW_ERR_INVALID;
+    o->requests = ctx->blocks->requests;
+    o->hit_blocks = ctx->blocks->hit_blocks;
+    o->miss_blocks = ctx->blocks->miss_blocks;
+    o->evictions = ctx->blocks->evictions;
+    o->trie_nodes = ctx->tree->nodes();
+    o->order_probes = ctx->tree->probes();
+    o->free_blocks = ctx->blocks->free_count();
+    o->seq = ctx->tree->seq();
+    return CW_OK;
+}
+
+// ---- ordering ---------------------------------------------------------------------------------------------
+static bool has_duplicates(const int64_t* ids, int32_t k) {
+    if (k <= 16) {
+        for (int i = 0; i < k; ++i)
+            for (int j = i + 1; j < k; ++j)
+                if (ids[i] == ids[j]) return true;
+        return false;
+    }
+    std::unordered_set<int64_t> s(ids, ids + k);
+    return (int32_t)s.size() != k;
+}
+
+int cw_order(cw_ctx* ctx, const int64_t* doc_ids, int32_t k, int64_t* out_order, int32_t* out_pred) {
+    if (!ctx || k < 0 || (k > 0 && (!doc_ids || !out_order))) return fail(ctx, CW_ERR_INVALID, "cw_order: bad argument");
+    if (has_duplicates(doc_ids, k)) return fail(ctx, CW_ERR_INVALID, "cw_order: duplicate document id");
+    int depth = ctx->tree->order(doc_ids, k, out_order);
+    if (out_pred) *out_pred = depth;
+    return CW_OK;
+}
+
+int cw_predict(cw_ctx* ctx, const int64_t* order, int32_t k, int32_t* out_prefix_docs) {
+    if (!ctx || k < 0 || (k > 0 && !order) || !out_prefix_docs) return fail(ctx, CW_ERR_INVALID, "cw_predict: bad argument");
+    *out_prefix_docs = ctx->tree->predict(order, k);
+    return CW_OK;
+}
+
+int cw_observe(cw_ctx* ctx, const int64_t* ordered, int32_t k) {
+    if (!ctx || k < 0 || (k > 0 && !ordered)) return fail(ctx, CW_ERR_INVALID, "cw_observe: bad argument");
+    if (has_duplicates(ordered, k)) return fail(ctx, CW_ERR_INVALID, "cw_observe: duplicate document id");
+    ctx->tree->observe(ordered, k);
+    return CW_OK;
+}
+
+// ---- prefix cache -----------------------------------------------------------------------------------------
+int cw_hash_chain(cw_ctx* ctx, const int32_t* tokens, int32_t n, uint64_t* out_chain) {
+    if (!ctx || n < 0 || (n > 0 && !tokens) || (n >= CW_BLOCK_SIZE && !out_chain))
+        return fail(ctx, CW_ERR_INVALID, "cw_hash_chain: bad argument");
+    std::vector<uint64_t> ch;
+    ctx->blocks->chain(tokens, n, ch);
+    if (!ch.empty()) std::memcpy(out_chain, ch.data(), ch.size() * sizeof(uint64_t));
+    return CW_OK;
+}
+
+int cw_lookup(cw_ctx* ctx, const int32_t* tokens, int32_t n, int32_t peek_only, int64_t* out_req,
+              int32_t* out_block_table, int32_t* out_n_cached) {
+    if (!ctx || !tokens || n <= 0 || !out_n_cached) return fail(ctx, CW_ERR_INVALID, "cw_lookup: bad argument");
+    if (peek_only) {
+        std::vector<uint64_t> ch;
+        ctx->blocks->chain(tokens, n, ch);
+        *out_n_cached = ctx->blocks->match(ch, n) * CW_BLOCK_SIZE;
+        return CW_OK;
+    }
+    if (!out_req || !out_block_table) return fail(ctx, CW_ERR_INVALID, "cw_lookup: null output");
+    return ctx->blocks->lookup(tokens, n, out_req, out_block_table, out_n_cached);
+}
+
+int cw_release(cw_ctx* ctx, int64_t req) {
+    if (!ctx) return CW_ERR_INVALID;
+    return ctx->blocks->release(req);
+}
+
+int cw_free_list(cw_ctx* ctx, int32_t* out, int32_t cap, int32_t* out_len) {
+    if (!ctx || !out_len || cap < 0 || (cap > 0 && !out)) return fail(ctx, CW_ERR_INVALID, "cw_free_list: bad argument");
+    *out_len = ctx->blocks->free_list(out, cap);
+    return CW_OK;
+}
+
+// ---- device work ------------------------------------------------------------------------------------------
+int cw_append_kv(cw_ctx* ctx, const void* q, const void* k, const void* v, void* q_roped, const int32_t* d_cu,
+                 const int32_t* d_nc, const int32_t* d_tables, int32_t max_blocks, int32_t B, int32_t T, void* stream) {
+    if (!ctx || ctx->host_only) return fail(ctx, CW_ERR_INVALID, "cw_append_kv: host-only context");
+    if (B < 0 || T < 0 || max_blocks <= 0) return fail(ctx, CW_ERR_INVALID, "cw_append_kv: bad sizes");
+    if (T == 0 || B == 0) return CW_OK;
+    if (!q || !k || !v || !q_roped || !d_cu || !d_nc || !d_tables || q == q_roped)
+        return fail(ctx, CW_ERR_INVALID, "cw_append_kv: null or aliased pointer");
+    int e = cw::launch_append_kv(ctx->cfg, q, k, v, q_roped, d_cu, d_nc, d_tables, max_blocks, B, T, stream);
+    return e ? cuda_fail(ctx, e, "cw_append_kv") : CW_OK;
+}
+
+int cw_gather_kv(cw_ctx* ctx, const int32_t* d_table, int32_t n, void* k_out, void* v_out, void* stream) {
+    if (!ctx || ctx->host_only) return fail(ctx, CW_ERR_INVALID, "cw_gather_kv: host-only context");
+    if (n < 0) return fail(ctx, CW_ERR_INVALID, "cw_gather_kv: bad size");
+    if (n == 0) return CW_OK;
+    if (!d_table || !k_out || !v_out) return fail(ctx, CW_ERR_INVALID, "cw_gather_kv: null pointer");
+    int e = cw::launch_gather_kv(ctx->cfg, d_table, n, k_out, v_out, stream);
+    return e ? cuda_fail(ctx, e, "cw_gather_kv") : CW_OK;
+}
+
+int64_t cw_attn_work_ints(cw_ctx* ctx, const int32_t* h_cu, int32_t B) {
+    if (!ctx || B < 0 || (B > 0 && !h_cu)) return CW_ERR_INVALID;
+    return 4 * cw::attn_count_tiles(ctx->cfg, h_cu, B);
+}
+
+int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out, const int32_t* h_cu, const int32_t* h_nc,
+                    const int32_t* d_cu, const int32_t* d_nc, const int32_t* d_tables, int32_t max_blocks, int32_t B,
+                    int32_t T, int32_t* d_work, void* stream) {
+    if (!ctx || ctx->host_only) return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn: host-only context");
+    if (B < 0 || T < 0 || max_blocks <= 0) return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn: bad sizes");
+    if (T == 0 || B == 0) return CW_OK;
+    if (!q_roped || !out || !h_cu || !h_nc || !d_cu || !d_nc || !d_tables || !d_work)
+        return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn: null pointer");
+    if (h_cu[0] != 0 || h_cu[B] != T) return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn: cu_seqlens_q does not span T");
+    for (int r = 0; r < B; ++r) {
+        const int s = h_cu[r + 1] - h_cu[r];
+        if (s < 0 || h_nc[r] < 0 || h_nc[r] % CW_BLOCK_SIZE != 0 ||
+            (int64_t)h_nc[r] + s > (int64_t)max_blocks * CW_BLOCK_SIZE || h_nc[r] + s > ctx->cfg.max_position)
+            return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn: bad request descriptor");
+    }
+    std::vector<int32_t> work;
+    const int64_t tiles = cw::attn_build_schedule(ctx->cfg, h_cu, h_nc, B, work);
+    if (tiles == 0) return CW_OK;
+    cudaError_t e = cudaMemcpyAsync(d_work, work.data(), work.size() * sizeof(int32_t), cudaMemcpyHostToDevice,
+                                    static_cast<cudaStream_t>(stream));   // pageable source: staged before return
+    if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_attn (schedule copy)");
+    int le = cw::launch_prefill_attn(ctx->cfg, q_roped, out, d_cu, d_nc, d_tables, max_blocks, d_work, tiles,
+                                     ctx->num_sms, stream);
+    return le ? cuda_fail(ctx, le, "cw_prefill_attn") : CW_OK;
+}
+
+// ---- host-buffer entry point ------------------------------------------------------------------------------
+namespace {
+struct WsLayout {
+    int64_t q, k, v, qr, out, cu, nc, tables, work, total;
+};
+WsLayout ws_layout(const cw_config& c, int32_t B, int32_t T, int32_t max_blocks) {
+    WsLayout w{};
+    const int64_t qb = (int64_t)T * c.num_q_heads * c.head_dim * 2, kb = (int64_t)T * c.num_kv_heads * c.head_dim * 2;
+    int64_t o = 0;
+    w.q = o; o += align256(qb);
+    w.k = o; o += align256(kb);
+    w.v = o; o += align256(kb);
+    w.qr = o; o += align256(qb);
+    w.out = o; o += align256(qb);
+    w.cu = o; o += align256((int64_t)(B + 1) * 4);
+    w.nc = o; o += align256((int64_t)B * 4);
+    w.tables = o; o += align256((int64_t)B * max_blocks * 4);
+    // upper bound on tiles: every request may add one ragged tile per kv head
+    const int g = c.num_q_heads / c.num_kv_heads;
+    const int64_t max_tiles = (((int64_t)T * g + 127) / 128 + B) * c.num_kv_heads;
+    w.work = o; o += align256(max_tiles * 16);
+    w.total = o;
+    return w;
+}
+}  // namespace
+
+int64_t cw_prefill_host_ws_bytes(cw_ctx* ctx, int32_t B, int32_t T, int32_t max_blocks) {
+    if (!ctx || B < 0 || T < 0 || max_blocks <= 0) return CW_ERR_INVALID;
+    return ws_layout(ctx->cfg, B, T, max_blocks).total;
+}
+
+int cw_prefill_host(cw_ctx* ctx, const void* h_q, const void* h_k, const void* h_v, void* h_out,
+                    const int32_t* h_cu, const int32_t* h_nc, const int32_t* h_tables, int32_t max_blocks, int32_t B,
+                    int32_t T, void* d_ws, void* stream) {
+    if (!ctx || ctx->host_only) return fail(ctx, CW_ERR_INVALID, "cw_prefill_host: host-only context");
+    if (B < 0 || T < 0 || max_blocks <= 0) return fail(ctx, CW_ERR_INVALID, "cw_prefill_host: bad sizes");
+    if (T == 0 || B == 0) return CW_OK;
+    if (!h_q || !h_k || !h_v || !h_out || !h_cu || !h_nc || !h_tables || !d_ws)
+        return fail(ctx, CW_ERR_INVALID, "cw_prefill_host: null pointer");
+    const cw_config& c = ctx->cfg;
+    const WsLayout w = ws_layout(c, B, T, max_blocks);
+    auto s = static_cast<cudaStream_t>(stream);
+    char* ws = static_cast<char*>(d_ws);
+    const size_t qb = (size_t)T * c.num_q_heads * c.head_dim * 2, kb = (size_t)T * c.num_kv_heads * c.head_dim * 2;
+    cudaError_t e = cudaMemcpyAsync(ws + w.q, h_q, qb, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ws + w.k, h_k, kb, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ws + w.v, h_v, kb, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ws + w.cu, h_cu, (size_t)(B + 1) * 4, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ws + w.nc, h_nc, (size_t)B * 4, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(ws + w.tables, h_tables, (size_t)B * max_blocks * 4, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_host (H2D)");
+    int rc = cw_append_kv(ctx, ws + w.q, ws + w.k, ws + w.v, ws + w.qr, (const int32_t*)(ws + w.cu),
+                          (const int32_t*)(ws + w.nc), (const int32_t*)(ws + w.tables), max_blocks, B, T, stream);
+    if (rc != CW_OK) return rc;
+    rc = cw_prefill_attn(ctx, ws + w.qr, ws + w.out, h_cu, h_nc, (const int32_t*)(ws + w.cu), (const int32_t*)(ws + w.nc),
+                         (const int32_t*)(ws + w.tables), max_blocks, B, T, (int32_t*)(ws + w.work), stream);
+    if (rc != CW_OK) return rc;
+    e = cudaMemcpyAsync(h_out, ws + w.out, qb, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_host (D2H)");
+    return CW_OK;
+}
+
+}  // extern "C"

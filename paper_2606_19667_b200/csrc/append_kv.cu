@@ -1,0 +1,155 @@
+// Kernel 1: fused RoPE + KV scatter (cw_append_kv) and the pool export kernel (cw_gather_kv).  sm_100a.
+//
+// For each suffix token at absolute position p (readings c4, §4):
+//     q_roped = RoPE(q, p);  pool_K[slot(p)] = RoPE(k, p);  pool_V[slot(p)] = v;  slot(p) = (table[p/16], p%16)
+// HBM-bound: every byte is read once and written once.  One CTA (128 threads) walks tokens grid-stride; inside a
+// token a thread owns "units" = one 16-byte chunk of the low half of a head plus its RoPE partner chunk in the
+// high half, so all global accesses are 16-byte vectors and 8 consecutive threads cover one full 128-byte line.
+// The pool block layout is the tcgen05 canonical 128B-swizzled tile (cacheweaver.h: cw_pool_offset).
+#include <cuda_bf16.h>
+#include <cuda_runtime.h>
+
+#include "cw_internal.h"
+
+namespace cw {
+
+__device__ __forceinline__ uint4 ld_stream(const void* p) {
+    uint4 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ void st_stream(void* p, const uint4& v) {
+    asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1,%2,%3,%4};"
+                 :: "l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
+
+__device__ __forceinline__ float2 bf2_to_f2(uint32_t u) {
+    return make_float2(__uint_as_float(u << 16), __uint_as_float(u & 0xFFFF0000u));
+}
+__device__ __forceinline__ uint32_t f2_to_bf2(float a, float b) {
+    __nv_bfloat162 h = __floats2bfloat162_rn(a, b);
+    return *reinterpret_cast<uint32_t*>(&h);
+}
+
+// rotate one (lo, hi) chunk pair: cs = 8 x {cos, sin} fp32 for the 8 frequencies of this chunk
+__device__ __forceinline__ void rope_pair(uint4& lo, uint4& hi, const float4* __restrict__ cs) {
+    uint32_t* l = reinterpret_cast<uint32_t*>(&lo);
+    uint32_t* h = reinterpret_cast<uint32_t*>(&hi);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        float4 t = __ldg(cs + j);                       // {cos0, sin0, cos1, sin1}
+        float2 a = bf2_to_f2(l[j]), b = bf2_to_f2(h[j]);
+        float x0 = a.x * t.x - b.x * t.y, y0 = b.x * t.x + a.x * t.y;
+        float x1 = a.y * t.z - b.y * t.w, y1 = b.y * t.z + a.y * t.w;
+        l[j] = f2_to_bf2(x0, x1);
+        h[j] = f2_to_bf2(y0, y1);
+    }
+}
+
+// element offset of dim d (multiple of 8) of token-in-block t inside one (block, kv head) run of 16*D elements
+template <int D>
+__device__ __forceinline__ int pool_chunk_offset(int t, int d) {
+    return (t >> 3) * (8 * D) + (d >> 6) * 512 + (t & 7) * 64 + ((((d & 63) >> 3) ^ (t & 7)) << 3);
+}
+
+template <int D>
+__global__ void __launch_bounds__(128) append_kv_kernel(
+    const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ k, const __nv_bfloat16* __restrict__ v,
+    __nv_bfloat16* __restrict__ q_roped, __nv_bfloat16* __restrict__ k_pool, __nv_bfloat16* __restrict__ v_pool,
+    const float* __restrict__ rope_table, const int32_t* __restrict__ cu, const int32_t* __restrict__ ncached,
+    const int32_t* __restrict__ tables, int max_blocks, int B, int T, int Hq, int Hkv, int max_position) {
+    constexpr int CPH = D / 16;                       // chunk pairs (units) per head
+    const int uq = Hq * CPH, uk = Hkv * CPH;
+    const int units = uq + 2 * uk;
+    for (int tok = blockIdx.x; tok < T; tok += gridDim.x) {
+        // request of this token: largest r with cu[r] <= tok
+        int lo = 0, hi = B;
+        while (hi - lo > 1) {
+            int mid = (lo + hi) >> 1;
+            if (__ldg(cu + mid) <= tok) lo = mid; else hi = mid;
+        }
+        const int r = lo;
+        int p = __ldg(ncached + r) + (tok - __ldg(cu + r));
+        const int blk = __ldg(tables + (size_t)r * max_blocks + (p >> 4));
+        const int tib = p & 15;
+        const int prow = p < max_position ? p : max_position - 1;
+        const float4* cs_row = reinterpret_cast<const float4*>(rope_table + (size_t)prow * D);
+        for (int u = threadIdx.x; u < units; u += 128) {
+            if (u < uq) {
+                const int h = u / CPH, c = u % CPH;
+                const size_t off = ((size_t)tok * Hq + h) * D + c * 8;
+                uint4 a = ld_stream(q + off), b = ld_stream(q + off + D / 2);
+                rope_pair(a, b, cs_row + c * 4);
+                st_stream(q_roped + off, a);
+                st_stream(q_roped + off + D / 2, b);
+            } else if (u < uq + uk) {
+                const int uu = u - uq, h = uu / CPH, c = uu % CPH;
+                const size_t off = ((size_t)tok * Hkv + h) * D + c * 8;
+                uint4 a = ld_stream(k + off), b = ld_stream(k + off + D / 2);
+                rope_pair(a, b, cs_row + c * 4);
+                __nv_bfloat16* base = k_pool + ((size_t)blk * Hkv + h) * (16 * D);
+                st_stream(base + pool_chunk_offset<D>(tib, c * 8), a);
+                st_stream(base + pool_chunk_offset<D>(tib, c * 8 + D / 2), b);
+            } else {
+                const int uu = u - uq - uk, h = uu / CPH, c = uu % CPH;
+                const size_t off = ((size_t)tok * Hkv + h) * D + c * 8;
+                uint4 a = ld_stream(v + off), b = ld_stream(v + off + D / 2);
+                __nv_bfloat16* base = v_pool + ((size_t)blk * Hkv + h) * (16 * D);
+                st_stream(base + pool_chunk_offset<D>(tib, c * 8), a);
+                st_stream(base + pool_chunk_offset<D>(tib, c * 8 + D / 2), b);
+            }
+        }
+    }
+}
+
+int launch_append_kv(const cw_config& cfg, const void* q, const void* k, const void* v, void* q_roped,
+                     const int32_t* cu, const int32_t* ncached, const int32_t* tables, int32_t max_blocks,
+                     int32_t B, int32_t T, void* stream) {
+    if (T == 0) return 0;
+    int grid = T < 148 * 16 ? T : 148 * 16;
+    auto s = static_cast<cudaStream_t>(stream);
+#define CW_LAUNCH_APPEND(DD)                                                                                    \
+    append_kv_kernel<DD><<<grid, 128, 0, s>>>(                                                                  \
+        (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, (__nv_bfloat16*)q_roped,     \
+        (__nv_bfloat16*)cfg.k_pool, (__nv_bfloat16*)cfg.v_pool, (const float*)cfg.rope_table, cu, ncached,      \
+        tables, max_blocks, B, T, cfg.num_q_heads, cfg.num_kv_heads, cfg.max_position)
+    if (cfg.head_dim == 128) CW_LAUNCH_APPEND(128); else CW_LAUNCH_APPEND(64);
+#undef CW_LAUNCH_APPEND
+    return (int)cudaGetLastError();
+}
+
+// ---- export: pool -> plain [n, Hkv, D] ---------------------------------------------------------------------
+template <int D>
+__global__ void __launch_bounds__(128) gather_kv_kernel(
+    const __nv_bfloat16* __restrict__ k_pool, const __nv_bfloat16* __restrict__ v_pool,
+    const int32_t* __restrict__ table, int n, int Hkv, __nv_bfloat16* __restrict__ k_out,
+    __nv_bfloat16* __restrict__ v_out) {
+    constexpr int CH = D / 8;
+    const int per_tok = Hkv * CH;
+    for (int tok = blockIdx.x; tok < n; tok += gridDim.x) {
+        const int blk = __ldg(table + (tok >> 4)), tib = tok & 15;
+        for (int u = threadIdx.x; u < per_tok; u += 128) {
+            const int h = u / CH, c = u % CH;
+            const size_t src = ((size_t)blk * Hkv + h) * (16 * D) + pool_chunk_offset<D>(tib, c * 8);
+            const size_t dst = ((size_t)tok * Hkv + h) * D + c * 8;
+            *reinterpret_cast<uint4*>(k_out + dst) = *reinterpret_cast<const uint4*>(k_pool + src);
+            *reinterpret_cast<uint4*>(v_out + dst) = *reinterpret_cast<const uint4*>(v_pool + src);
+        }
+    }
+}
+
+int launch_gather_kv(const cw_config& cfg, const int32_t* table, int32_t n, void* k_out, void* v_out, void* stream) {
+    if (n == 0) return 0;
+    int grid = n < 148 * 8 ? n : 148 * 8;
+    auto s = static_cast<cudaStream_t>(stream);
+    if (cfg.head_dim == 128)
+        gather_kv_kernel<128><<<grid, 128, 0, s>>>((const __nv_bfloat16*)cfg.k_pool, (const __nv_bfloat16*)cfg.v_pool,
+                                                   table, n, cfg.num_kv_heads, (__nv_bfloat16*)k_out, (__nv_bfloat16*)v_out);
+    else
+        gather_kv_kernel<64><<<grid, 128, 0, s>>>((const __nv_bfloat16*)cfg.k_pool, (const __nv_bfloat16*)cfg.v_pool,
+                                                  table, n, cfg.num_kv_heads, (__nv_bfloat16*)k_out, (__nv_bfloat16*)v_out);
+    return (int)cudaGetLastError();
+}
+
+}  // namespace cw

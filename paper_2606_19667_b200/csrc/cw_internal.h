@@ -1,0 +1,116 @@
+// Internal declarations shared by the host state (host.cpp), the kernels (*.cu) and the C ABI (api.cu).
+// Product code: nothing here is shared with oracle/.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <unordered_map>
+#include <vector>
+
+#include "cacheweaver.h"
+
+namespace cw {
+
+// ---- knowledge tree (§3.2) -------------------------------------------------------------------
+// Flat representation: one hash map keyed by (parent node id, doc id).  A path stamps every node on it with
+// the same seq, so last_seq(child) <= last_seq(parent): a stale parent has only stale children and nodes can
+// be pruned individually (result-invariant, "bounded by the recency window").
+struct TrieKey {
+    uint64_t parent;
+    int64_t doc;
+    bool operator==(const TrieKey& o) const { return parent == o.parent && doc == o.doc; }
+};
+struct TrieKeyHash {
+    size_t operator()(const TrieKey& k) const {
+        uint64_t x = k.parent * 0x9E3779B97F4A7C15ull ^ (uint64_t)k.doc * 0xC2B2AE3D27D4EB4Full;
+        x ^= x >> 29;
+        return (size_t)(x * 0xBF58476D1CE4E5B9ull);
+    }
+};
+struct TrieNode {
+    uint64_t id;
+    int64_t last_seq;
+};
+
+class KnowledgeTree {
+  public:
+    explicit KnowledgeTree(int64_t window) : H_(window) {}
+    // Algorithm 1.  Returns depth l(O,T).
+    int order(const int64_t* D, int k, int64_t* O);
+    int predict(const int64_t* O, int k) const;
+    void observe(const int64_t* O, int k);
+    int64_t nodes() const { return (int64_t)map_.size(); }
+    int64_t probes() const { return probes_; }
+    int64_t seq() const { return seq_; }
+
+  private:
+    const TrieNode* child(uint64_t parent, int64_t doc) const;
+    bool cached(const TrieNode* n) const { return seq_ - n->last_seq < H_; }
+    void prune();
+    std::unordered_map<TrieKey, TrieNode, TrieKeyHash> map_;
+    int64_t H_;
+    int64_t seq_ = 0;
+    int64_t last_prune_ = 0;
+    uint64_t next_id_ = 1;  // 0 = root
+    int64_t probes_ = 0;
+};
+
+// ---- paged KV block manager (reading c3) --------------------------------
+struct Request {
+    std::vector<int32_t> table;
+    std::vector<uint64_t> chain;
+    int32_t m;
+};
+
+class BlockManager {
+  public:
+    BlockManager(int32_t num_blocks, bool eager, uint64_t salt);
+    void chain(const int32_t* tokens, int32_t n, std::vector<uint64_t>& out) const;
+    int32_t match(const std::vector<uint64_t>& chain, int32_t n) const;
+    // returns CW_OK / CW_ERR_NO_SPACE
+    int lookup(const int32_t* tokens, int32_t n, int64_t* req, int32_t* table, int32_t* n_cached);
+    int release(int64_t req);
+    int32_t free_list(int32_t* out, int32_t cap) const;
+    int64_t requests = 0, hit_blocks = 0, miss_blocks = 0, evictions = 0;
+    int32_t free_count() const { return free_count_; }
+
+  private:
+    void unlink(int32_t b);
+    void push_tail(int32_t b);
+    void reg(const Request& r, int32_t nfull);
+    int32_t NB_;
+    bool eager_;
+    uint64_t salt_;
+    std::vector<int32_t> ref_, prev_, next_;   // list nodes 0..NB-1, sentinel = NB
+    std::vector<uint8_t> has_hash_;
+    std::vector<uint64_t> hash_;
+    std::unordered_map<uint64_t, int32_t> index_;
+    std::unordered_map<int64_t, Request> reqs_;
+    int64_t next_req_ = 1;
+    int32_t free_count_;
+};
+
+}  // namespace cw
+
+struct cw_ctx {
+    cw_config cfg;
+    cw::KnowledgeTree* tree;
+    cw::BlockManager* blocks;
+    std::string last_error;
+    bool host_only;
+    int num_sms;
+};
+
+// kernel launchers (defined in the .cu files); return cudaError_t as int
+namespace cw {
+int launch_append_kv(const cw_config& cfg, const void* q, const void* k, const void* v, void* q_roped,
+                     const int32_t* cu, const int32_t* ncached, const int32_t* tables, int32_t max_blocks,
+                     int32_t B, int32_t T, void* stream);
+int launch_gather_kv(const cw_config& cfg, const int32_t* table, int32_t n, void* k_out, void* v_out, void* stream);
+// tile schedule: 4 ints per tile {request, kv_head, first packed row, num kv tokens}; returns tile count
+int64_t attn_count_tiles(const cw_config& cfg, const int32_t* h_cu, int32_t B);
+int64_t attn_build_schedule(const cw_config& cfg, const int32_t* h_cu, const int32_t* h_nc, int32_t B,
+                            std::vector<int32_t>& work);
+int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* cu,
+                        const int32_t* ncached, const int32_t* tables, int32_t max_blocks, const int32_t* d_work,
+                        int64_t num_tiles, int num_sms, void* stream);
+}  // namespace cw

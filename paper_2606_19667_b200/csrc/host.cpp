@@ -1,0 +1,195 @@
+// Host state of the prefix-cached prefill path: knowledge tree + greedy ordering and the
+// paged-KV block manager with chained block hashes and LRU eviction (DESIGN.md c2, c3).
+// Product code; shares nothing with oracle/.
+#include "cw_internal.h"
+
+#include <algorithm>
+#include <cstring>
+
+namespace cw {
+
+// ------------------------------------------------------------------------------------------------ trie ----
+const TrieNode* KnowledgeTree::child(uint64_t parent, int64_t doc) const {
+    auto it = map_.find(TrieKey{parent, doc});
+    return it == map_.end() ? nullptr : &it->second;
+}
+
+// Algorithm 1.  R is kept as an index list in retrieval rank; "for each d in R" scans it in that order and takes
+// the first cached child (DESIGN.md reading: D is given in retrieval rank).
+int KnowledgeTree::order(const int64_t* D, int k, int64_t* O) {
+    std::vector<int64_t> R(D, D + k);                 // line 1: O <- [], R <- D, node <- root
+    uint64_t node = 0;
+    int n_out = 0;
+    probes_ = 0;
+    while (!R.empty()) {                              // line 2
+        bool found = false;                           // line 3
+        for (size_t i = 0; i < R.size(); ++i) {       // line 4
+            ++probes_;
+            const TrieNode* c = child(node, R[i]);    // line 5
+            if (c && cached(c)) {                     // line 6
+                O[n_out++] = R[i];                    // line 7: append d to O, remove d from R
+                R.erase(R.begin() + (long)i);
+                node = c->id;                         // line 8
+                found = true;
+                break;
+            }
+        }
+        if (!found) {                                 // lines 11-13: remaining R in retrieval-rank order
+            for (int64_t d : R) O[n_out++] = d;
+            break;
+        }
+    }
+    return predict(O, k);
+}
+
+int KnowledgeTree::predict(const int64_t* O, int k) const {
+    uint64_t node = 0;
+    int m = 0;
+    for (; m < k; ++m) {
+        const TrieNode* c = child(node, O[m]);
+        if (!c || !cached(c)) break;
+        node = c->id;
+    }
+    return m;
+}
+
+void KnowledgeTree::observe(const int64_t* O, int k) {
+    ++seq_;
+    uint64_t node = 0;
+    for (int i = 0; i < k; ++i) {
+        TrieKey key{node, O[i]};
+        auto it = map_.find(key);
+        if (it == map_.end()) it = map_.emplace(key, TrieNode{next_id_++, seq_}).first;
+        it->second.last_seq = seq_;
+        node = it->second.id;
+    }
+    if (seq_ - last_prune_ >= std::max<int64_t>(H_, 16)) prune();
+}
+
+void KnowledgeTree::prune() {
+    last_prune_ = seq_;
+    for (auto it = map_.begin(); it != map_.end();) {
+        if (seq_ - it->second.last_seq >= H_) it = map_.erase(it);
+        else ++it;
+    }
+}
+
+// --------------------------------------------------------------------------------------- block manager ----
+static inline uint64_t fnv1a_step(uint64_t h, uint8_t byte) { return (h ^ byte) * 0x100000001B3ull; }
+
+BlockManager::BlockManager(int32_t num_blocks, bool eager, uint64_t salt)
+    : NB_(num_blocks), eager_(eager), salt_(salt), ref_(num_blocks, 0), prev_(num_blocks + 1), next_(num_blocks + 1),
+      has_hash_(num_blocks, 0), hash_(num_blocks, 0), free_count_(num_blocks) {
+    // circular list with sentinel NB: head = next_[NB], tail = prev_[NB]; initial order 0,1,...,NB-1
+    for (int32_t b = 0; b <= NB_; ++b) {
+        next_[b] = (b + 1) % (NB_ + 1);
+        prev_[b] = (b + NB_) % (NB_ + 1);
+    }
+    index_.reserve((size_t)num_blocks * 2);
+}
+
+void BlockManager::unlink(int32_t b) {
+    next_[prev_[b]] = next_[b];
+    prev_[next_[b]] = prev_[b];
+    --free_count_;
+}
+
+void BlockManager::push_tail(int32_t b) {
+    int32_t t = prev_[NB_];
+    next_[t] = b; prev_[b] = t; next_[b] = NB_; prev_[NB_] = b;
+    ++free_count_;
+}
+
+// h_i = FNV1a64(LE64(h_{i-1}) || LE32(tok[16i]) ... LE32(tok[16i+15])), h_{-1} = salt  (DESIGN.md c2)
+void BlockManager::chain(const int32_t* tokens, int32_t n, std::vector<uint64_t>& out) const {
+    int32_t nfull = n / CW_BLOCK_SIZE;
+    out.resize((size_t)nfull);
+    uint64_t parent = salt_;
+    for (int32_t i = 0; i < nfull; ++i) {
+        uint64_t h = 0xCBF29CE484222325ull;
+        for (int b = 0; b < 8; ++b) h = fnv1a_step(h, (uint8_t)(parent >> (8 * b)));
+        for (int t = 0; t < CW_BLOCK_SIZE; ++t) {
+            uint32_t tok = (uint32_t)tokens[i * CW_BLOCK_SIZE + t];
+            for (int b = 0; b < 4; ++b) h = fnv1a_step(h, (uint8_t)(tok >> (8 * b)));
+        }
+        out[(size_t)i] = parent = h;
+    }
+}
+
+int32_t BlockManager::match(const std::vector<uint64_t>& ch, int32_t n) const {
+    int32_t cap = (n - 1) / CW_BLOCK_SIZE, m = 0;
+    while (m < cap && index_.count(ch[(size_t)m])) ++m;
+    return m;
+}
+
+void BlockManager::reg(const Request& r, int32_t nfull) {
+    for (int32_t i = r.m; i < nfull; ++i) {
+        auto ins = index_.emplace(r.chain[(size_t)i], r.table[(size_t)i]);
+        if (ins.second) {
+            has_hash_[(size_t)r.table[(size_t)i]] = 1;
+            hash_[(size_t)r.table[(size_t)i]] = r.chain[(size_t)i];
+        }
+    }
+}
+
+int BlockManager::lookup(const int32_t* tokens, int32_t n, int64_t* req, int32_t* table, int32_t* n_cached) {
+    Request r;
+    chain(tokens, n, r.chain);
+    int32_t nblk = (n + CW_BLOCK_SIZE - 1) / CW_BLOCK_SIZE, nfull = n / CW_BLOCK_SIZE;
+    r.m = match(r.chain, n);                                                    // (1)
+    r.table.resize((size_t)nblk);
+    int32_t matched_free = 0;
+    for (int32_t i = 0; i < r.m; ++i) {
+        int32_t b = index_.find(r.chain[(size_t)i])->second;
+        r.table[(size_t)i] = b;
+        if (ref_[(size_t)b] == 0) ++matched_free;
+    }
+    if (nblk - r.m > free_count_ - matched_free) return CW_ERR_NO_SPACE;        // (2) nothing changed so far
+    for (int32_t i = 0; i < r.m; ++i) {                                         // (3) pin the hit blocks
+        int32_t b = r.table[(size_t)i];
+        if (ref_[(size_t)b] == 0) unlink(b);
+        ++ref_[(size_t)b];
+    }
+    for (int32_t i = r.m; i < nblk; ++i) {                                      // (4) pop head, evict its hash
+        int32_t b = next_[NB_];
+        unlink(b);
+        if (has_hash_[(size_t)b]) {
+            index_.erase(hash_[(size_t)b]);
+            has_hash_[(size_t)b] = 0;
+            ++evictions;
+        }
+        ref_[(size_t)b] = 1;
+        r.table[(size_t)i] = b;
+    }
+    if (eager_) reg(r, nfull);                                                  // (5)
+    std::memcpy(table, r.table.data(), sizeof(int32_t) * (size_t)nblk);
+    *n_cached = r.m * CW_BLOCK_SIZE;
+    *req = next_req_++;
+    ++requests; hit_blocks += r.m; miss_blocks += nblk - r.m;
+    reqs_.emplace(*req, std::move(r));
+    return CW_OK;
+}
+
+int BlockManager::release(int64_t req) {
+    auto it = reqs_.find(req);
+    if (it == reqs_.end()) return CW_ERR_BAD_HANDLE;
+    Request& r = it->second;
+    if (!eager_) reg(r, (int32_t)r.chain.size());
+    for (int32_t i = (int32_t)r.table.size() - 1; i >= 0; --i) {               // reverse: deepest evicted first
+        int32_t b = r.table[(size_t)i];
+        if (--ref_[(size_t)b] == 0) push_tail(b);
+    }
+    reqs_.erase(it);
+    return CW_OK;
+}
+
+int32_t BlockManager::free_list(int32_t* out, int32_t cap) const {
+    int32_t n = 0;
+    for (int32_t b = next_[NB_]; b != NB_; b = next_[b]) {
+        if (n < cap) out[n] = b;
+        ++n;
+    }
+    return n;
+}
+
+}  // namespace cw
