@@ -1,0 +1,219 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI (ctypes binding), against the fp64 oracle
+on the same seeded inputs, element by element.
+
+Bars (BASELINE.json north_star): bit-exact for orders / block tables / n_cached; RoPE'd bf16 values within
+1 bf16 ulp of the fp64 result; attention outputs max|d| <= 2e-2 and ||d||2/||ref||2 <= 1e-2 against the fp64 oracle.
+"""
+import numpy as np
+import pytest
+
+import tracegen
+from oracle import attention as oattn
+from oracle.pipeline import full_recompute, run_trace
+from paper_2606_19667_b200 import Context, CwError
+from paper_2606_19667_b200.engine import TraceRunner
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+MAX_ABS, REL_L2 = 2e-2, 1e-2          # north_star tolerances for bf16 attention outputs
+
+
+@pytest.fixture(scope="module")
+def dev():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    return "cuda:0"
+
+
+def to_dev(bits: np.ndarray, dev):
+    return torch.from_numpy(np.ascontiguousarray(bits).view(np.int16)).view(torch.bfloat16).to(dev)
+
+
+def to_bits(t) -> np.ndarray:
+    return t.contiguous().view(torch.int16).cpu().numpy().view(np.uint16)
+
+
+def rand_bits(rng, *shape):
+    return tracegen.f32_to_bf16_bits(rng.standard_normal(shape, dtype=np.float32))
+
+
+def assert_close_attn(got_bits, ref, what=""):
+    got = tracegen.bf16_bits_to_f64(got_bits).reshape(ref.shape)
+    d = got - ref
+    max_abs = float(np.abs(d).max())
+    rel = float(np.linalg.norm(d) / np.linalg.norm(ref))
+    assert np.isfinite(got).all(), f"{what}: non-finite output"
+    assert max_abs <= MAX_ABS and rel <= REL_L2, f"{what}: max_abs={max_abs:.3e} rel_l2={rel:.3e}"
+    return max_abs, rel
+
+
+def assert_bf16_ulp(got_bits, ref, what=""):
+    """|got - ref| <= 1 bf16 ulp of ref (ulp <= 2^-7 |ref|), plus the subnormal floor."""
+    got = tracegen.bf16_bits_to_f64(got_bits).reshape(ref.shape)
+    err = np.abs(got - ref)
+    bound = np.abs(ref) * 2.0 ** -7 + 1e-30
+    bad = err > bound
+    assert not bad.any(), f"{what}: {bad.sum()} elements off by more than 1 bf16 ulp (max err {err.max():.3e})"
+
+
+class Batch:
+    """Hand-built varlen batch: request r has n_cached c[r] (multiple of 16) and suffix length s[r]; block tables are
+    a seeded permutation of the pool.  The prefix K/V is written by a first cw_append_kv call with c = 0."""
+
+    def __init__(self, dev, Hq, Hkv, D, cs, ss, theta=5e5, seed=0, NB=None):
+        rng = np.random.default_rng(seed)
+        self.dev, self.Hq, self.Hkv, self.D, self.theta = dev, Hq, Hkv, D, theta
+        self.cs, self.ss = list(cs), list(ss)
+        self.B = len(cs)
+        self.ns = [c + s for c, s in zip(cs, ss)]
+        nblk = [-(-n // 16) for n in self.ns]
+        self.max_blocks = max(nblk)
+        NB = NB or sum(nblk) + 3
+        perm = rng.permutation(NB).astype(np.int32)
+        self.tables = np.zeros((self.B, self.max_blocks), dtype=np.int32)
+        o = 0
+        for r in range(self.B):
+            self.tables[r, :nblk[r]] = perm[o:o + nblk[r]]
+            o += nblk[r]
+        self.q = [rand_bits(rng, n, Hq, D) for n in self.ns]
+        self.k = [rand_bits(rng, n, Hkv, D) for n in self.ns]
+        self.v = [rand_bits(rng, n, Hkv, D) for n in self.ns]
+        self.ctx = Context(NB, Hq, Hkv, D, 4, rope_theta=theta, max_position=max(self.ns), device=dev)
+        self.d_tables = torch.from_numpy(self.tables).to(dev)
+
+    def _append(self, lo, hi):
+        """append positions lo[r]..hi[r]-1 of every request (rows with hi==lo contribute nothing)."""
+        lens = [h - l for l, h in zip(lo, hi)]
+        cu = np.zeros(self.B + 1, dtype=np.int32)
+        cu[1:] = np.cumsum(lens)
+        T = int(cu[-1])
+        cat = lambda xs: np.concatenate([x[l:h] for x, l, h in zip(xs, lo, hi)], axis=0)
+        q, k, v = (to_dev(cat(x), self.dev) for x in (self.q, self.k, self.v))
+        qr = torch.empty_like(q)
+        d_cu = torch.from_numpy(cu).to(self.dev)
+        nc = np.asarray(lo, dtype=np.int32)
+        d_nc = torch.from_numpy(nc).to(self.dev)
+        self.ctx.cw_append_kv(q, k, v, qr, d_cu, d_nc, self.d_tables, self.max_blocks, self.B, T)
+        return qr, cu, nc, d_cu, d_nc, T
+
+    def run(self):
+        if any(self.cs):
+            self._append([0] * self.B, self.cs)
+        qr, cu, nc, d_cu, d_nc, T = self._append(self.cs, self.ns)
+        out = torch.full_like(qr, float("nan"))
+        d_work = torch.empty(max(4, self.ctx.cw_attn_work_ints(cu)), dtype=torch.int32, device=self.dev)
+        self.ctx.cw_prefill_attn(qr, out, cu, nc, d_cu, d_nc, self.d_tables, self.max_blocks, self.B, T, d_work)
+        torch.cuda.synchronize()
+        return to_bits(qr), to_bits(out), cu
+
+    def oracle(self, r):
+        f = tracegen.bf16_bits_to_f64
+        return oattn.attention_full(f(self.q[r]), f(self.k[r]), f(self.v[r]), self.theta)[self.cs[r]:]
+
+
+# ---- kernel 1: fused RoPE + KV scatter --------------------------------------------------------------------
+@pytest.mark.parametrize("Hq,Hkv,D", [(2, 1, 64), (32, 8, 128), (28, 4, 128)])
+def test_append_kv_pool_contents_and_q_roped(dev, Hq, Hkv, D):
+    b = Batch(dev, Hq, Hkv, D, cs=[0, 32, 16], ss=[37, 5, 130], seed=1)
+    qr_bits, _, cu = b.run()
+    f = tracegen.bf16_bits_to_f64
+    for r in range(b.B):
+        n, c = b.ns[r], b.cs[r]
+        pos = np.arange(n)
+        k_ref = oattn.rope(f(b.k[r]), pos, b.theta)
+        q_ref = oattn.rope(f(b.q[r]), pos, b.theta)[c:]
+        assert_bf16_ulp(qr_bits[cu[r]:cu[r + 1]], q_ref, f"q_roped r={r}")
+        k_out = torch.empty(n, Hkv, D, dtype=torch.bfloat16, device=dev)
+        v_out = torch.empty_like(k_out)
+        d_table = torch.from_numpy(b.tables[r]).to(dev)
+        b.ctx.cw_gather_kv(d_table, n, k_out, v_out)
+        torch.cuda.synchronize()
+        assert_bf16_ulp(to_bits(k_out), k_ref, f"pool K r={r}")
+        assert np.array_equal(to_bits(v_out), b.v[r]), "pool V must be a bit-exact copy"
+        # the documented pool layout (cw_pool_offset) addresses the same elements
+        kp = to_bits(b.ctx.k_pool)
+        for (p, h, d) in [(0, 0, 0), (n - 1, Hkv - 1, D - 1), (n // 2, 0, D // 2 + 3), (17 % n, Hkv - 1, 9)]:
+            off = b.ctx.cw_pool_offset(int(b.tables[r, p // 16]), h, p % 16, d)
+            assert kp[off] == to_bits(k_out)[p, h, d]
+
+
+def test_append_kv_position_zero_is_identity(dev):
+    b = Batch(dev, 4, 2, 128, cs=[0], ss=[1], seed=2)
+    qr_bits, out_bits, _ = b.run()
+    assert np.array_equal(qr_bits[0], b.q[0][0])            # RoPE at p = 0 is the identity
+    # row p = 0 attends only key 0: o = v_0 exactly (bit-exact bf16)
+    g = 2
+    for h in range(4):
+        assert np.array_equal(out_bits[0, h], b.v[0][0, h // g])
+
+
+# ---- kernel 2: varlen paged causal GQA attention ----------------------------------------------------------
+@pytest.mark.parametrize("Hq,Hkv,D,cs,ss", [
+    (2, 1, 64, [0], [224]),                                  # cfg-1 shape, cold
+    (2, 1, 64, [64, 0, 192], [160, 1, 32]),                  # cfg-1 shape, cached prefixes, 1-row request
+    (32, 8, 128, [0, 256], [300, 48 + 256]),                 # 8B shape, several tiles + ragged tails
+    (32, 8, 128, [1280], [48]),                              # query-only suffix after a long hit
+    (28, 4, 128, [512, 0], [77, 129]),                       # Qwen shape, g = 7 (rows of a head straddle tiles)
+    (64, 8, 128, [128], [200]),                              # 70B shape, g = 8
+])
+def test_attention_matches_oracle(dev, Hq, Hkv, D, cs, ss):
+    b = Batch(dev, Hq, Hkv, D, cs, ss, seed=3)
+    _, out_bits, cu = b.run()
+    for r in range(b.B):
+        assert_close_attn(out_bits[cu[r]:cu[r + 1]], b.oracle(r), f"r={r} c={cs[r]} s={ss[r]}")
+
+
+def test_attention_constant_v_and_zero_q(dev):
+    """V == const => o == const; Q == 0 => o = running mean of V."""
+    b = Batch(dev, 8, 2, 128, cs=[0], ss=[300], seed=4)
+    b.q[0][:] = 0
+    _, out_bits, _ = b.run()
+    v = tracegen.bf16_bits_to_f64(b.v[0])
+    mean = np.cumsum(v, axis=0) / np.arange(1, 301)[:, None, None]
+    ref = np.repeat(mean, 4, axis=1)
+    assert_close_attn(out_bits, ref, "running mean")
+
+
+def test_empty_batch_and_bad_descriptors(dev):
+    b = Batch(dev, 2, 1, 64, cs=[0], ss=[20], seed=5)
+    z = torch.zeros(4, dtype=torch.int32, device=dev)
+    e = torch.empty(0, 2, 64, dtype=torch.bfloat16, device=dev)
+    b.ctx.cw_append_kv(e, e, e, e, z, z, z, 1, 0, 0)                           # B = T = 0: OK, no launch
+    b.ctx.cw_prefill_attn(e, e, np.zeros(1, np.int32), np.zeros(0, np.int32), z, z, z, 1, 0, 0, z)
+    q = torch.zeros(20, 2, 64, dtype=torch.bfloat16, device=dev)
+    with pytest.raises(CwError):                                               # n_cached not a multiple of 16
+        b.ctx.cw_prefill_attn(q, torch.empty_like(q), np.array([0, 20], np.int32), np.array([8], np.int32),
+                              z, z, b.d_tables, b.max_blocks, 1, 20, z)
+    with pytest.raises(CwError):                                               # q_roped aliases q
+        b.ctx.cw_append_kv(q, q, q, q, z, z, b.d_tables, b.max_blocks, 1, 20)
+
+
+# ---- whole path on the BASELINE.json traces ---------------------------------------------------------------
+@pytest.mark.parametrize("strategy", ["greedy", "retrieval"])
+def test_trace_cfg1_all_rows(dev, strategy):
+    trace = tracegen.make_trace(tracegen.CONFIGS[1])
+    ref = run_trace(trace, strategy)
+    run = TraceRunner(trace, strategy, device=dev)
+    recs = run.run()
+    assert len(recs) == len(ref.requests)
+    for a, o in zip(recs, ref.requests):
+        assert a.order == o.order and a.depth == o.depth and a.n_cached == o.n_cached
+        assert a.table.tolist() == list(o.table)
+        assert_close_attn(a.out, o.out, f"cfg1 {strategy} r={a.r}")
+        # prefix-cached == full recompute of the same ordered prompt
+        assert_close_attn(a.out, full_recompute(trace, o)[o.n_cached:], f"cfg1 {strategy} r={a.r} vs full")
+
+
+def test_trace_cfg2_first_requests_all_rows(dev):
+    """8B shape, first 6 requests of config 2 (the oracle needs ~2 s per cold request)."""
+    trace = tracegen.make_trace(tracegen.CONFIGS[2])
+    reqs = list(range(6))
+    ref = run_trace(trace, "greedy", requests=reqs)
+    recs = TraceRunner(trace, "greedy", device=dev).run(requests=reqs)
+    hits = 0
+    for a, o in zip(recs, ref.requests):
+        assert a.order == o.order and a.n_cached == o.n_cached and a.table.tolist() == list(o.table)
+        assert_close_attn(a.out, o.out, f"cfg2 r={a.r} c={a.n_cached}")
+        hits += a.n_cached
+    assert hits > 0, "the greedy arm must reuse some prefix on config 2"
