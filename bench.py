@@ -1,0 +1,428 @@
+"""bench.py — prefix-cached prefill (CacheWeaver hot path) on B200, one process per GPU.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--impl ours|reference]
+
+A *step* is one pass of the whole hot path over one batch of synthetic input: the requests
+of the configuration are admitted on the host in ONE cw_admit_batch call on a reset context (greedy trie order,
+prompt assembly, chained block hashes, prefix match, pin/allocate/evict, trie insert), then ONE cw_append_kv launch
+(fused RoPE + KV scatter) and ONE cw_prefill_attn launch (varlen paged causal GQA attention) over all suffixes,
+then cw_release_batch.  Workload at N=1: BASELINE.json configs[1] (Llama-3-8B-shaped layer, 64 requests, 200x256-token
+documents, top-k 5, 60 % adjacent overlap, 8192-block pool).  Metric: attention TFLOP/s over algorithmic flops
+4*Hq*D*[n(n+1)/2 - c(c+1)/2] per request (BASELINE.json `metric`), plus batch prefill ms for greedy vs retrieval order.
+The path does not shard (BASELINE.json north_star: one GPU): --gpus N runs N independent replicas ("replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import tracegen  # noqa: E402
+
+METRIC = "prefill-attn TFLOP/s (% bf16 peak); batch prefill ms, greedy vs retrieval order"
+UNIT = "TFLOP/s"
+
+
+def attention_flops(cfg, n_cached):
+    n = cfg.n
+    return sum(4 * cfg.Hq * cfg.D * (n * (n + 1) // 2 - int(c) * (int(c) + 1) // 2) for c in n_cached)
+
+
+def append_bytes(cfg, T):
+    """algorithmic bytes of cw_append_kv: q in + q' out + k,v in + pool K,V out + 4 B descriptor per token."""
+    return int(T) * (2 * cfg.Hq * cfg.D * 2 + 2 * 2 * cfg.Hkv * cfg.D * 2 + 4)
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return {"bf16": float(d["bf16_tflops"]), "bf16_sustained": float(d.get("bf16_tflops_sustained", d["bf16_tflops"])),
+                "hbm": float(d["hbm_gbs"]), "source": "measured (MEASURED_PEAKS.json, burst)"}
+    return {"bf16": 1590.0, "bf16_sustained": 1400.0, "hbm": 6650.0, "source": "fallback (B200_PROFILING.md)"}
+
+
+def traffic_from_profile(kernel):
+    """dram bytes per launch from the committed ncu summary (profiles/traffic.json), else None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        return json.load(open(p)).get(kernel)
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            time.sleep(0.06)
+            self.proc.terminate()
+            self.t.join(timeout=2)
+
+    def summary(self):
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for nm, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ---------------------------------------------------------------------------------------------- our arm ----
+class Workload:
+    """One configuration, one strategy: seeded trace, resident inputs, and the step function."""
+    RING = 4
+
+    def __init__(self, cfg_id, strategy, device, want_e2e=True):
+        import torch
+        from paper_2606_19667_b200.engine import admit_waves, make_context
+        self.torch, self.device, self.strategy = torch, device, strategy
+        self.cfg = cfg = tracegen.CONFIGS[cfg_id] if isinstance(cfg_id, int) else cfg_id
+        self.trace = trace = tracegen.make_trace(cfg)
+        self.ctx = make_context(cfg, device)
+        self.doc_ids = np.asarray(trace.retrieval, dtype=np.int64)
+        # dry admission (host only) fixes the wave boundaries and suffix descriptors; every step repeats it for real
+        self.waves = admit_waves(self.ctx, trace, strategy)
+        self.ctx.cw_reset()
+        self.flops = sum(attention_flops(cfg, w.nc) for w in self.waves)
+        self.T = sum(w.T for w in self.waves)
+        self.hit_blocks = sum(int(w.nc.sum()) // 16 for w in self.waves)
+        self.max_blocks = cfg.blocks_per_req
+        Bmax = max(w.B for w in self.waves)
+        self.inputs, self.host_inputs = [], []
+        for w in self.waves:
+            rows = tracegen.batch_suffix_qkv(trace, w.items, threads=os.cpu_count() or 8)
+            qkv = [torch.from_numpy(x.view(np.int16)).view(torch.bfloat16) for x in tracegen.split_qkv(cfg, rows)]
+            if want_e2e:
+                self.host_inputs.append([t.pin_memory() for t in qkv] + [torch.empty_like(qkv[0]).pin_memory()])
+            dq, dk, dv = (t.to(device) for t in qkv)
+            work = torch.empty(max(4, self.ctx.cw_attn_work_ints(w.cu)), dtype=torch.int32, device=device)
+            self.inputs.append((dq, dk, dv, torch.empty_like(dq), torch.empty_like(dq), work))
+        # pinned staging ring for the admission outputs + device descriptors
+        self.ring = []
+        for _ in range(self.RING):
+            # Bmax + 1 rows: the request that closes a wave (CW_ERR_NO_SPACE) still gets its order written
+            st = {"orders": torch.empty(Bmax + 1, cfg.k, dtype=torch.int64).pin_memory(),
+                  "pred": torch.empty(Bmax + 1, dtype=torch.int32).pin_memory(),
+                  "reqs": torch.empty(Bmax + 1, dtype=torch.int64).pin_memory(),
+                  "tables": torch.empty(Bmax + 1, self.max_blocks, dtype=torch.int32).pin_memory(),
+                  "n_cached": torch.empty(Bmax + 1, dtype=torch.int32).pin_memory(),
+                  "cu": torch.empty(Bmax + 2, dtype=torch.int32).pin_memory()}
+            st["np"] = {k: v.numpy() for k, v in st.items()}
+            st["d_tables"] = torch.empty(Bmax, self.max_blocks, dtype=torch.int32, device=device)
+            st["d_nc"] = torch.empty(Bmax, dtype=torch.int32, device=device)
+            st["d_cu"] = torch.empty(Bmax + 1, dtype=torch.int32, device=device)
+            st["event"] = None
+            self.ring.append(st)
+        self.slot, self.Bmax = 0, Bmax
+        self.ws = None
+        if want_e2e:
+            nbytes = max(self.ctx.cw_prefill_host_ws_bytes(w.B, w.T, self.max_blocks) for w in self.waves)
+            self.ws = torch.empty(nbytes, dtype=torch.uint8, device=device)
+        self.queries = np.ascontiguousarray(trace.query_tokens)
+        self.launches = 0
+        self.h2d = self.d2h = 0
+
+    def _admit(self, lo, expect):
+        st = self.ring[self.slot]
+        self.slot = (self.slot + 1) % self.RING
+        if st["event"] is not None:
+            st["event"].synchronize()
+        hi = lo + self.Bmax + 1
+        a = self.ctx.cw_admit_batch(self.doc_ids[lo:hi], self.strategy == "greedy", self.trace.doc_tokens,
+                                    self.queries[lo:hi], self.max_blocks, out=st["np"])
+        if a["admitted"] != expect.B:
+            raise RuntimeError(f"admission diverged: {a['admitted']} != {expect.B}")
+        return st, a
+
+    def step(self, events=None):
+        """resident inputs: host admission + H2D of the descriptors + 2 launches per wave."""
+        torch, ctx = self.torch, self.ctx
+        ctx.cw_reset()
+        lo = 0
+        for wi, w in enumerate(self.waves):
+            st, a = self._admit(lo, w)
+            B, T = w.B, w.T
+            st["d_tables"][:B].copy_(st["tables"][:B], non_blocking=True)
+            st["d_nc"][:B].copy_(st["n_cached"][:B], non_blocking=True)
+            st["d_cu"][:B + 1].copy_(st["cu"][:B + 1], non_blocking=True)
+            q, k, v, qr, out, work = self.inputs[wi]
+            if events is not None:
+                e = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+                e[0].record()
+            ctx.cw_append_kv(q, k, v, qr, st["d_cu"], st["d_nc"], st["d_tables"], self.max_blocks, B, T)
+            if events is not None:
+                e[1].record()
+            ctx.cw_prefill_attn(qr, out, a["cu"], a["n_cached"], st["d_cu"], st["d_nc"], st["d_tables"], self.max_blocks,
+                                B, T, work)
+            if events is not None:
+                e[2].record()
+                events.append(e)
+            st["event"] = torch.cuda.Event()
+            st["event"].record()
+            ctx.cw_release_batch(a["reqs"][:B])
+            self.launches += 2
+            lo += B
+
+    def step_e2e(self):
+        """host buffers: admission + cw_prefill_host (H2D of q,k,v and descriptors, both kernels, D2H of out)."""
+        ctx = self.ctx
+        ctx.cw_reset()
+        lo = 0
+        for wi, w in enumerate(self.waves):
+            st, a = self._admit(lo, w)
+            hq, hk, hv, hout = self.host_inputs[wi]
+            ctx.cw_prefill_host(hq, hk, hv, hout, a["cu"], a["n_cached"], a["tables"][:w.B], self.max_blocks, w.B, w.T, self.ws)
+            ctx.cw_release_batch(a["reqs"][:w.B])
+            self.h2d += (hq.numel() + hk.numel() + hv.numel()) * 2 + 4 * (2 * w.B + 1 + w.B * self.max_blocks)
+            self.d2h += hout.numel() * 2
+            lo += w.B
+        return hout
+
+
+# --------------------------------------------------------------------------------------- oracle timing ----
+def oracle_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [p.get("num_threads", 1) for p in threadpool_info()]
+        return max(n) if n else 1
+    except Exception:
+        return 1
+
+
+class OracleSample:
+    """The oracle as it stands (oracle/, fp64 numpy), timed on a bounded sample: the first `n_req` requests of the
+    configuration, greedy order, sequential: order/lookup/observe + RoPE + pool append + suffix attention + release.
+    Inputs are generated before the timed region."""
+
+    def __init__(self, cfg_id, n_req):
+        from oracle.pipeline import run_trace
+        self.cfg = cfg = tracegen.CONFIGS[cfg_id]
+        self.trace = tracegen.make_trace(cfg)
+        self.reqs = list(range(min(n_req, cfg.n_req)))
+        dry = run_trace(self.trace, "greedy", compute=False, requests=self.reqs)
+        self.flops = attention_flops(cfg, [rr.n_cached for rr in dry.requests])
+        for rr in dry.requests:                       # warm tracegen's chunk cache: no RNG inside the timed region
+            tracegen.prompt_qkv(self.trace, rr.r, rr.order, rr.n_cached, cache=True)
+        self.dry = dry
+
+    def run(self):
+        from oracle.attention import PagedPool, attention_suffix
+        from oracle.blocks import BlockManager
+        from oracle.ordering import KnowledgeTree
+        cfg, trace = self.cfg, self.trace
+        t0 = time.perf_counter()
+        tree, bm, pool = KnowledgeTree(cfg.H), BlockManager(cfg.NB, eager_register=True), PagedPool(cfg.NB, cfg.Hkv, cfg.D)
+        for r in self.reqs:
+            O, _ = tree.order(trace.retrieval[r])
+            tokens = tracegen.assemble_prompt(trace, r, O)
+            req, table, c = bm.lookup(tokens)
+            tree.observe(O)
+            rows = tracegen.prompt_qkv(trace, r, O, c, cache=True)
+            q, k, v = (tracegen.bf16_bits_to_f64(x) for x in tracegen.split_qkv(cfg, rows))
+            attention_suffix(pool, table, c, q, k, v, cfg.theta)
+            bm.release(req)
+        return time.perf_counter() - t0
+
+
+# ------------------------------------------------------------------------------------------------ main ----
+def dist_env():
+    return int(os.environ.get("RANK", 0)), int(os.environ.get("LOCAL_RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the box's host cores (rank 0 only), same metric / unit / config."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    sample = OracleSample(args.config, args.oracle_requests)
+    for _ in range(args.warmup):
+        sample.run()
+    times = [sample.run() for _ in range(args.steps)]
+    total = sum(times)
+    value = sample.flops * args.steps / total / 1e12
+    cores = oracle_threads()
+    desc = f"first {len(sample.reqs)} of {sample.cfg.n_req} requests of {sample.cfg.name} per step, sequential, greedy order"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({sample.cfg.name})", "sample": desc},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def timed(torch, fn, steps, dist):
+    """barrier + sync, K steps, sync; device time by CUDA events on the launching (current) stream; max over ranks."""
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+        dist.barrier()
+    return ms
+
+
+def run_ours(args):
+    import torch
+    rank, local, world = dist_env()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback")
+    torch.cuda.set_device(local)
+    device = f"cuda:{local}"
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device(device))
+    pk = peaks()
+    wl = Workload(args.config, "greedy", device)
+    cfg = wl.cfg
+
+    for _ in range(args.warmup):
+        wl.step()
+    wl.launches = 0
+    events = []
+    with ClockSampler(local) as clk:
+        ms = timed(torch, lambda: wl.step(events), args.steps, dist)
+    launches = wl.launches
+    ms_step = ms / args.steps
+    value = world * wl.flops / (ms_step * 1e-3) / 1e12
+    app_ms = sum(e[0].elapsed_time(e[1]) for e in events) / args.steps       # per step, all waves
+    attn_ms = sum(e[1].elapsed_time(e[2]) for e in events) / args.steps
+    n_l = len(wl.waves)
+    attn_tflops = wl.flops / (attn_ms * 1e-3) / 1e12
+    app_gbs = append_bytes(cfg, wl.T) / (app_ms * 1e-3) / 1e9
+
+    # end to end: host buffers, H2D/D2H inside the timed region
+    for _ in range(max(1, args.warmup // 2)):
+        wl.step_e2e()
+    wl.h2d = wl.d2h = 0
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    ms_e2e = timed(torch, wl.step_e2e, e2e_steps, dist) / e2e_steps
+    e2e_value = world * wl.flops / (ms_e2e * 1e-3) / 1e12
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    # second half of the metric: batch prefill ms, greedy vs retrieval order (same trace, fresh context)
+    prefill = {"greedy": {"ms": app_ms + attn_ms, "append_ms": app_ms, "attn_ms": attn_ms, "suffix_tokens": wl.T,
+                          "hit_blocks": wl.hit_blocks, "attn_flops": wl.flops}}
+    if not args.skip_retrieval:
+        del wl.host_inputs, wl.ws
+        wr = Workload(args.config, "retrieval", device, want_e2e=False)
+        for _ in range(args.warmup):
+            wr.step()
+        ev = []
+        timed(torch, lambda: wr.step(ev), args.steps, None)
+        r_app = sum(e[0].elapsed_time(e[1]) for e in ev) / args.steps
+        r_attn = sum(e[1].elapsed_time(e[2]) for e in ev) / args.steps
+        prefill["retrieval"] = {"ms": r_app + r_attn, "append_ms": r_app, "attn_ms": r_attn, "suffix_tokens": wr.T,
+                                "hit_blocks": wr.hit_blocks, "attn_flops": wr.flops}
+        prefill["ratio_measured"] = prefill["greedy"]["ms"] / prefill["retrieval"]["ms"]
+        prefill["ratio_predicted_by_flops"] = wl.flops / wr.flops
+        del wr
+
+    cpu = None
+    if world == 1 or rank == 0:
+        sample = OracleSample(args.config, args.oracle_requests)
+        t = sample.run()
+        desc = f"first {len(sample.reqs)} of {cfg.n_req} requests of {cfg.name}, sequential, greedy order, one pass"
+        cpu = {"value": sample.flops / t / 1e12, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle", "sample": desc,
+               "seconds": t}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+            "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({cfg.name})", "requests": cfg.n_req,
+                       "prompt_tokens": cfg.n, "heads": f"{cfg.Hq}q/{cfg.Hkv}kv x {cfg.D}", "pool_blocks": cfg.NB,
+                       "admission": f"one varlen wave per launch ({n_l} wave(s)), eager block registration",
+                       "order": "greedy", "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "l2": "inputs larger than L2 (q,k,v,pool >> 126 MB per step); no explicit flush"},
+            "pct_of_bf16_peak": 100.0 * value / world / pk["bf16"],
+            "clocks": clk.summary(),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": wl.h2d // e2e_steps,
+                    "d2h_bytes_per_step": wl.d2h // e2e_steps, "ms_per_step": ms_e2e, "steps": e2e_steps},
+            "gpu_launches": launches,
+            "roofline": {"kernel": "prefill_attn_kernel", "bound": "tensor", "achieved": attn_tflops, "peak": pk["bf16"],
+                         "unit": "TFLOP/s", "frac": attn_tflops / pk["bf16"], "traffic": traffic_from_profile("prefill_attn_kernel"),
+                         "peak_source": pk["source"], "frac_of_sustained": attn_tflops / pk["bf16_sustained"],
+                         "flops_per_step": wl.flops, "avg_ms": attn_ms / n_l, "launches_per_step": n_l},
+            "roofline_append_kv": {"kernel": "append_kv_kernel", "bound": "hbm", "achieved": app_gbs, "peak": pk["hbm"],
+                                   "unit": "GB/s", "frac": app_gbs / pk["hbm"], "traffic": traffic_from_profile("append_kv_kernel"),
+                                   "bytes_per_step": append_bytes(cfg, wl.T), "avg_ms": app_ms / n_l},
+            "batch_prefill": prefill,
+            "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--oracle-requests", type=int, default=None, help="requests in the oracle's bounded sample")
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--skip-retrieval", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.oracle_requests is None:
+        args.oracle_requests = {1: 4, 2: 16 if args.impl == "ours" else 4, 4: 1, 5: 1}[args.config]
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -101,6 +101,28 @@ int cw_lookup(cw_ctx* ctx, const int32_t* tokens, int32_t n, int32_t peek_only,
               int64_t* out_req, int32_t* out_block_table, int32_t* out_n_cached);
 /* Unpin; blocks whose refcount reaches 0 go to the LRU tail in REVERSE block order. */
 int cw_release(cw_ctx* ctx, int64_t req);
+/* Back to the state right after cw_create: empty knowledge tree, empty prefix index, LRU list 0..NB-1, no live
+ * requests, statistics zeroed.  Pools and the RoPE table are untouched (old KV is unreachable: nothing is indexed). */
+int cw_reset(cw_ctx* ctx);
+/* Admission of a wave in ONE call: steps a1..a6 (+a2) for requests r = 0..B-1, in order (DESIGN.md reading
+ * "requests of a batch are admitted sequentially on the host"):
+ *     O_r = reorder ? Algorithm1(doc_ids[r]) : doc_ids[r];                      (cw_order / cw_predict)
+ *     tokens = doc_tokens[O_r[0]] || ... || doc_tokens[O_r[k-1]] || query_tokens[r];   (prompt assembly)
+ *     (req, table, n_cached) = cw_lookup(tokens);  cw_observe(O_r)
+ * All pointers HOST.  doc_ids [B,k] in retrieval rank; doc_tokens [num_docs, doc_len]; query_tokens [B, q_len];
+ * out_orders [B,k]; out_pred_prefix_docs [B]; out_reqs [B]; out_block_tables [B, max_blocks] (unused tail entries
+ * are set to 0; max_blocks >= ceil((k*doc_len+q_len)/16)); out_n_cached [B]; out_cu_seqlens_q [B+1] (prefix sums of
+ * the suffix lengths n - n_cached).  Admission stops at the first request that does not fit (CW_ERR_NO_SPACE; that
+ * request and all later ones leave the state unchanged); *out_admitted = number admitted, return value CW_OK unless
+ * an argument is invalid (doc id outside [0,num_docs), duplicate ids, ...), in which case admission also stops. */
+int cw_admit_batch(cw_ctx* ctx, const int64_t* doc_ids, int32_t B, int32_t k, int32_t reorder,
+                   const int32_t* doc_tokens, int32_t num_docs, int32_t doc_len,
+                   const int32_t* query_tokens, int32_t q_len,
+                   int64_t* out_orders, int32_t* out_pred_prefix_docs, int64_t* out_reqs,
+                   int32_t* out_block_tables, int32_t max_blocks, int32_t* out_n_cached,
+                   int32_t* out_cu_seqlens_q, int32_t* out_admitted);
+/* cw_release for reqs[0..B-1] in order; stops at the first bad handle. */
+int cw_release_batch(cw_ctx* ctx, const int64_t* reqs, int32_t B);
 /* Copy the LRU free list head->tail into out[cap] (host); returns its length via *out_len (testing aid). */
 int cw_free_list(cw_ctx* ctx, int32_t* out, int32_t cap, int32_t* out_len);
 

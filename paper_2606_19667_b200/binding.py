@@ -70,6 +70,10 @@ def load_library(build_if_missing: bool = True):
         "cw_lookup": (C.c_int, [vp, p(i32), i32, i32, p(i64), p(i32), p(i32)]),
         "cw_release": (C.c_int, [vp, i64]),
         "cw_free_list": (C.c_int, [vp, p(i32), i32, p(i32)]),
+        "cw_reset": (C.c_int, [vp]),
+        "cw_admit_batch": (C.c_int, [vp, p(i64), i32, i32, i32, p(i32), i32, i32, p(i32), i32, p(i64), p(i32), p(i64),
+                                     p(i32), i32, p(i32), p(i32), p(i32)]),
+        "cw_release_batch": (C.c_int, [vp, p(i64), i32]),
         "cw_append_kv": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp]),
         "cw_attn_work_ints": (i64, [vp, p(i32), i32]),
         "cw_prefill_attn": (C.c_int, [vp, vp, vp, p(i32), p(i32), vp, vp, vp, i32, i32, i32, vp, vp]),
@@ -86,6 +90,7 @@ def load_library(build_if_missing: bool = True):
 
 EXPORTS = ["cw_create", "cw_destroy", "cw_strerror", "cw_last_error", "cw_stats", "cw_pool_bytes", "cw_pool_offset",
            "cw_order", "cw_predict", "cw_observe", "cw_hash_chain", "cw_lookup", "cw_release", "cw_free_list",
+           "cw_reset", "cw_admit_batch", "cw_release_batch",
            "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_gather_kv", "cw_prefill_host_ws_bytes",
            "cw_prefill_host"]
 
@@ -192,6 +197,36 @@ class Context:
 
     def cw_release(self, req):
         self._check(self.lib.cw_release(self.h, req))
+
+    def cw_reset(self):
+        self._check(self.lib.cw_reset(self.h))
+
+    def cw_admit_batch(self, doc_ids, reorder, doc_tokens, query_tokens, max_blocks=None, out=None):
+        """doc_ids int64 [B,k]; doc_tokens int32 [num_docs, doc_len]; query_tokens int32 [B, q_len] (C-contiguous numpy).
+        Returns dict(orders, pred, reqs, tables, n_cached, cu, admitted); `out` may carry preallocated arrays."""
+        doc_ids = np.ascontiguousarray(doc_ids, dtype=np.int64)
+        doc_tokens, query_tokens = _np_i32(doc_tokens), _np_i32(query_tokens)
+        B, k = doc_ids.shape
+        num_docs, doc_len = doc_tokens.shape
+        q_len = query_tokens.shape[1]
+        if max_blocks is None:
+            max_blocks = -(-(k * doc_len + q_len) // BLOCK_SIZE)
+        o = out or {}
+        orders = o.get("orders", np.empty((B, k), dtype=np.int64))
+        pred = o.get("pred", np.empty(B, dtype=np.int32))
+        reqs = o.get("reqs", np.empty(B, dtype=np.int64))
+        tables = o.get("tables", np.empty((B, max_blocks), dtype=np.int32))
+        nc = o.get("n_cached", np.empty(B, dtype=np.int32))
+        cu = o.get("cu", np.empty(B + 1, dtype=np.int32))
+        adm = C.c_int32()
+        self._check(self.lib.cw_admit_batch(self.h, _i64p(doc_ids), B, k, int(bool(reorder)), _i32p(doc_tokens), num_docs,
+                                            doc_len, _i32p(query_tokens), q_len, _i64p(orders), _i32p(pred), _i64p(reqs),
+                                            _i32p(tables), max_blocks, _i32p(nc), _i32p(cu), C.byref(adm)))
+        return dict(orders=orders, pred=pred, reqs=reqs, tables=tables, n_cached=nc, cu=cu, admitted=adm.value)
+
+    def cw_release_batch(self, reqs):
+        r = np.ascontiguousarray(reqs, dtype=np.int64)
+        self._check(self.lib.cw_release_batch(self.h, _i64p(r), len(r)))
 
     def cw_free_list(self):
         out = np.empty(self.NB, dtype=np.int32)

@@ -1,6 +1,7 @@
 // C ABI of libcacheweaver.so (include/cacheweaver.h): argument checking, error mapping and glue only.
 #include <cuda_runtime.h>
 
+#include <climits>
 #include <cmath>
 #include <cstring>
 #include <new>
@@ -172,6 +173,69 @@ int cw_lookup(cw_ctx* ctx, const int32_t* tokens, int32_t n, int32_t peek_only, 
 int cw_release(cw_ctx* ctx, int64_t req) {
     if (!ctx) return CW_ERR_INVALID;
     return ctx->blocks->release(req);
+}
+
+int cw_reset(cw_ctx* ctx) {
+    if (!ctx) return CW_ERR_INVALID;
+    delete ctx->tree;
+    delete ctx->blocks;
+    ctx->tree = new cw::KnowledgeTree(ctx->cfg.recency_window);
+    ctx->blocks = new cw::BlockManager(ctx->cfg.num_blocks, ctx->cfg.eager_register != 0, ctx->cfg.hash_salt);
+    ctx->last_error.clear();
+    return CW_OK;
+}
+
+int cw_admit_batch(cw_ctx* ctx, const int64_t* doc_ids, int32_t B, int32_t k, int32_t reorder, const int32_t* doc_tokens,
+                   int32_t num_docs, int32_t doc_len, const int32_t* query_tokens, int32_t q_len, int64_t* out_orders,
+                   int32_t* out_pred, int64_t* out_reqs, int32_t* out_tables, int32_t max_blocks, int32_t* out_nc,
+                   int32_t* out_cu, int32_t* out_admitted) {
+    if (!ctx || B < 0 || k < 0 || doc_len < 0 || q_len < 0 || num_docs < 0 || !out_admitted || !out_cu)
+        return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: bad argument");
+    *out_admitted = 0;
+    out_cu[0] = 0;
+    if (B == 0) return CW_OK;
+    const int64_t n64 = (int64_t)k * doc_len + q_len;
+    if (n64 <= 0 || n64 > INT32_MAX || (n64 + CW_BLOCK_SIZE - 1) / CW_BLOCK_SIZE > max_blocks)
+        return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: prompt length / max_blocks");
+    if ((k > 0 && (!doc_ids || !doc_tokens || !out_orders)) || (q_len > 0 && !query_tokens) || !out_pred || !out_reqs ||
+        !out_tables || !out_nc)
+        return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: null pointer");
+    const int32_t n = (int32_t)n64, nblk = (n + CW_BLOCK_SIZE - 1) / CW_BLOCK_SIZE;
+    std::vector<int32_t> tokens((size_t)n);
+    for (int32_t r = 0; r < B; ++r) {
+        const int64_t* D = doc_ids + (size_t)r * k;
+        int64_t* O = out_orders + (size_t)r * k;
+        for (int i = 0; i < k; ++i)
+            if (D[i] < 0 || D[i] >= num_docs) return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: doc id out of range");
+        if (has_duplicates(D, k)) return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: duplicate document id");
+        if (reorder) {
+            out_pred[r] = ctx->tree->order(D, k, O);
+        } else {
+            std::memcpy(O, D, sizeof(int64_t) * (size_t)k);
+            out_pred[r] = ctx->tree->predict(O, k);
+        }
+        for (int i = 0; i < k; ++i)
+            std::memcpy(tokens.data() + (size_t)i * doc_len, doc_tokens + (size_t)O[i] * doc_len, sizeof(int32_t) * (size_t)doc_len);
+        if (q_len) std::memcpy(tokens.data() + (size_t)k * doc_len, query_tokens + (size_t)r * q_len, sizeof(int32_t) * (size_t)q_len);
+        int32_t* table = out_tables + (size_t)r * max_blocks;
+        int rc = ctx->blocks->lookup(tokens.data(), n, out_reqs + r, table, out_nc + r);
+        if (rc == CW_ERR_NO_SPACE) return CW_OK;
+        if (rc != CW_OK) return rc;
+        for (int32_t i = nblk; i < max_blocks; ++i) table[i] = 0;
+        ctx->tree->observe(O, k);
+        out_cu[r + 1] = out_cu[r] + (n - out_nc[r]);
+        *out_admitted = r + 1;
+    }
+    return CW_OK;
+}
+
+int cw_release_batch(cw_ctx* ctx, const int64_t* reqs, int32_t B) {
+    if (!ctx || B < 0 || (B > 0 && !reqs)) return fail(ctx, CW_ERR_INVALID, "cw_release_batch: bad argument");
+    for (int32_t i = 0; i < B; ++i) {
+        int rc = ctx->blocks->release(reqs[i]);
+        if (rc != CW_OK) return rc;
+    }
+    return CW_OK;
 }
 
 int cw_free_list(cw_ctx* ctx, int32_t* out, int32_t cap, int32_t* out_len) {

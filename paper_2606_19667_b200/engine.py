@@ -161,3 +161,34 @@ class TraceRunner:
             for b, rec in enumerate(wave.recs):
                 rec.out = o[wave.cu[b]: wave.cu[b + 1]]
         return q_roped, out
+
+
+def admit_waves(ctx: Context, trace: tracegen.Trace, strategy: str = "greedy", requests=None, on_wave=None,
+                force_waves: bool = True):
+    """Whole-trace admission through cw_admit_batch (one C call per wave) + cw_release_batch.
+    Admission "waves" (or force_waves): as many requests as fit are admitted, the wave is handed to on_wave (which
+    launches the kernels), released, and admission resumes.  Admission "sequential": one request per wave.
+    Returns the list of Wave objects (recs hold order / depth / table / n_cached, tokens omitted)."""
+    cfg = trace.cfg
+    todo = list(range(cfg.n_req)) if requests is None else list(requests)
+    doc_ids = np.asarray([trace.retrieval[r] for r in todo], dtype=np.int64).reshape(len(todo), cfg.k)
+    queries = np.ascontiguousarray(trace.query_tokens[todo])
+    waves, i = [], 0
+    step = None if (force_waves or cfg.admission == "waves") else 1
+    while i < len(todo):
+        j = len(todo) if step is None else min(len(todo), i + step)
+        a = ctx.cw_admit_batch(doc_ids[i:j], strategy == "greedy", trace.doc_tokens, queries[i:j], cfg.blocks_per_req)
+        m = a["admitted"]
+        if m == 0:
+            raise NoSpace(-2, "a single request does not fit the pool")
+        recs = [RequestRecord(todo[i + b], a["orders"][b].tolist(), int(a["pred"][b]), None,
+                              a["tables"][b, : cfg.blocks_per_req].copy(), int(a["n_cached"][b]), len(waves))
+                for b in range(m)]
+        wave = Wave([(rec.r, rec.order, rec.n_cached) for rec in recs], a["cu"][: m + 1].copy(), a["n_cached"][:m].copy(),
+                    a["tables"][:m].copy(), recs)
+        if on_wave is not None:
+            on_wave(wave)
+        ctx.cw_release_batch(a["reqs"][:m])
+        waves.append(wave)
+        i += m
+    return waves

@@ -221,3 +221,43 @@ def test_greedy_hits_at_least_retrieval_on_cfg2():
         runner = TraceRunner(tracegen.make_trace(cfg), s, ctx=make_context(cfg))
         hit[s] = sum(r.n_cached for r in runner.run(compute=False))
     assert hit["greedy"] > hit["retrieval"]
+
+
+@pytest.mark.parametrize("cfg_id,strategy", [(1, "greedy"), (2, "retrieval"), (4, "greedy"), (5, "greedy"), (5, "retrieval")])
+def test_admit_batch_equals_per_request_calls_and_oracle(cfg_id, strategy):
+    """cw_admit_batch (one C call per wave) == cw_order/cw_lookup/cw_observe per request == the oracle."""
+    from paper_2606_19667_b200.engine import admit_waves
+    cfg = tracegen.CONFIGS[cfg_id]
+    trace = tracegen.make_trace(cfg)
+    ref = run_trace(trace, strategy, compute=False)
+    ctx = make_context(cfg)
+    for _ in range(2):                                   # second pass after cw_reset must reproduce the first
+        waves = admit_waves(ctx, trace, strategy, force_waves=False)
+        recs = [rec for w in waves for rec in w.recs]
+        assert len(waves) == ref.waves and len(recs) == len(ref.requests)
+        for a, b in zip(recs, ref.requests):
+            assert (a.r, a.order, a.depth, a.n_cached, a.wave) == (b.r, b.order, b.depth, b.n_cached, b.wave)
+            assert a.table.tolist() == b.table
+        for w in waves:
+            assert w.cu[-1] == sum(cfg.n - c for c in w.nc) and w.cu[0] == 0
+        assert ctx.cw_stats()["evictions"] == ref.evictions
+        ctx.cw_reset()
+        st = ctx.cw_stats()
+        assert (st["requests"], st["trie_nodes"], st["free_blocks"], st["seq"]) == (0, 0, cfg.NB, 0)
+        assert ctx.cw_free_list() == list(range(cfg.NB))
+
+
+def test_admit_batch_invalid_arguments():
+    ctx = host_ctx(NB=64)
+    docs = np.zeros((4, 32), dtype=np.int32)
+    q = np.zeros((1, 8), dtype=np.int32)
+    with pytest.raises(CwError):
+        ctx.cw_admit_batch(np.array([[0, 9]]), True, docs, q)          # doc id out of range
+    with pytest.raises(CwError):
+        ctx.cw_admit_batch(np.array([[1, 1]]), True, docs, q)          # duplicate ids
+    with pytest.raises(CwError):
+        ctx.cw_admit_batch(np.array([[0, 1]]), True, docs, q, max_blocks=2)   # table too narrow
+    a = ctx.cw_admit_batch(np.array([[0, 1]]), True, docs, q)
+    assert a["admitted"] == 1 and a["cu"].tolist() == [0, 72]
+    with pytest.raises(CwError):
+        ctx.cw_release_batch([a["reqs"][0], 12345])
