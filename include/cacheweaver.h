@@ -78,6 +78,15 @@ int64_t cw_pool_bytes(const cw_config* cfg);
  *   off = ((block*Hkv + kv_head) * 16*D) + (t/8)*(8*D) + (d/64)*512 + (t%8)*64 + ((((d%64)/8) ^ (t%8))*8) + d%8 */
 int64_t cw_pool_offset(const cw_config* cfg, int32_t block, int32_t kv_head, int32_t t, int32_t d);
 
+/* element offset (bf16 elements, relative to the request's first element q_begin*Hq*D) of (suffix token tok, query
+ * head, dim d) inside q_roped, for a request with s suffix tokens.  q_roped is the intermediate between cw_append_kv
+ * and cw_prefill_attn and is stored TILE-PACKED so that the attention kernel loads a Q tile with one bulk copy per
+ * 64-dim half and feeds it to the MMA without re-layout.  With g = Hq/Hkv, tpt = 128/g tokens per tile:
+ *   kvh = head/g, t = tok/tpt, row = (tok%tpt)*g + head%g, rows = min(tpt, s - t*tpt)*g
+ *   off = kvh*s*g*D + t*(tpt*g)*D + (d/64)*rows*64 + row*64 + ((((d%64)/8) ^ (row%8))*8) + d%8
+ * i.e. a permutation of the request's own [s, Hq, D] slice. */
+int64_t cw_q_roped_offset(const cw_config* cfg, int32_t s, int32_t tok, int32_t head, int32_t d);
+
 /* ---- ordering, host (PAPER.md:57 knowledge tree; Algorithm 1) ------------------------- */
 /* Algorithm 1: doc_ids[k] in retrieval rank (host, distinct) -> out_order[k] (host); *out_pred_prefix_docs =
  * l(O,T), the depth of the cached trie path followed.  k == 0 is OK (empty order).
@@ -134,7 +143,8 @@ int cw_free_list(cw_ctx* ctx, int32_t* out, int32_t cap, int32_t* out_len);
  * cw_append_kv — fused RoPE + KV scatter (kernel 1):  for each suffix token at position p
  *     q_roped = RoPE(q, p);  pool_K[slot(p)] = RoPE(k, p);  pool_V[slot(p)] = v;
  *     slot(p) = (block_table[p/16], p%16)          (DESIGN.md c4 split-half RoPE)
- *   q [T,Hq,D], k,v [T,Hkv,D], q_roped [T,Hq,D]: device bf16, row-major contiguous; q_roped must NOT alias q
+ *   q [T,Hq,D], k,v [T,Hkv,D]: device bf16, row-major contiguous.  q_roped: device bf16, T*Hq*D elements, request r
+ *   owns the slice starting at cu_seqlens_q[r]*Hq*D, laid out as cw_q_roped_offset() says; it must NOT alias q
  *   (q is read through the non-coherent path).  Positions >= max_position are invalid.  The pools must have been
  *   zero-filled once by the caller (stale slots of a partially filled block must hold finite values). */
 int cw_append_kv(cw_ctx* ctx, const void* q, const void* k, const void* v, void* q_roped,
@@ -147,7 +157,7 @@ int cw_append_kv(cw_ctx* ctx, const void* q, const void* k, const void* v, void*
  *   h_cu_seqlens_q [B+1], h_n_cached [B]: HOST copies of the same descriptors (used only to build the tile
  *   schedule on the host; kv_len[r] = n_cached[r] + suffix length).  d_work: DEVICE int32 scratch of
  *   cw_attn_work_ints(...) ints, caller-owned, filled asynchronously on `stream` by this call.
- *   q_roped, out [T,Hq,D] device bf16. */
+ *   q_roped: as written by cw_append_kv (tile-packed); out [T,Hq,D] device bf16 row-major.  One persistent CTA per SM. */
 int64_t cw_attn_work_ints(cw_ctx* ctx, const int32_t* h_cu_seqlens_q, int32_t B);
 int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out,
                     const int32_t* h_cu_seqlens_q, const int32_t* h_n_cached,

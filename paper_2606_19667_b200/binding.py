@@ -63,6 +63,7 @@ def load_library(build_if_missing: bool = True):
         "cw_stats": (C.c_int, [vp, p(CwStats)]),
         "cw_pool_bytes": (i64, [p(CwConfig)]),
         "cw_pool_offset": (i64, [p(CwConfig), i32, i32, i32, i32]),
+        "cw_q_roped_offset": (i64, [p(CwConfig), i32, i32, i32, i32]),
         "cw_order": (C.c_int, [vp, p(i64), i32, p(i64), p(i32)]),
         "cw_predict": (C.c_int, [vp, p(i64), i32, p(i32)]),
         "cw_observe": (C.c_int, [vp, p(i64), i32]),
@@ -88,7 +89,7 @@ def load_library(build_if_missing: bool = True):
     return lib
 
 
-EXPORTS = ["cw_create", "cw_destroy", "cw_strerror", "cw_last_error", "cw_stats", "cw_pool_bytes", "cw_pool_offset",
+EXPORTS = ["cw_create", "cw_destroy", "cw_strerror", "cw_last_error", "cw_stats", "cw_pool_bytes", "cw_pool_offset", "cw_q_roped_offset",
            "cw_order", "cw_predict", "cw_observe", "cw_hash_chain", "cw_lookup", "cw_release", "cw_free_list",
            "cw_reset", "cw_admit_batch", "cw_release_batch",
            "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_gather_kv", "cw_prefill_host_ws_bytes",
@@ -241,6 +242,9 @@ class Context:
 
     def cw_pool_offset(self, block, kv_head, t, d):
         return self.lib.cw_pool_offset(C.byref(self.cfg), block, kv_head, t, d)
+
+    def cw_q_roped_offset(self, s, tok, head, d):
+        return self.lib.cw_q_roped_offset(C.byref(self.cfg), s, tok, head, d)
 
     # ---- device work ----
     @staticmethod

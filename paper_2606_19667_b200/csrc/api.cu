@@ -1,6 +1,7 @@
 // C ABI of libcacheweaver.so (include/cacheweaver.h): argument checking, error mapping and glue only.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <climits>
 #include <cmath>
 #include <cstring>
@@ -21,7 +22,8 @@ int cuda_fail(cw_ctx* ctx, int cuda_err, const char* where) {
 }
 bool bad_cfg(const cw_config* c) {
     return !c || c->block_size != CW_BLOCK_SIZE || c->num_blocks <= 0 || c->num_q_heads <= 0 || c->num_kv_heads <= 0 ||
-           c->num_q_heads % c->num_kv_heads != 0 || (c->head_dim != 64 && c->head_dim != 128) || c->recency_window <= 0;
+           c->num_q_heads % c->num_kv_heads != 0 || (c->head_dim != 64 && c->head_dim != 128) || c->recency_window <= 0 ||
+           c->num_q_heads / c->num_kv_heads > 128;
 }
 inline int64_t align256(int64_t x) { return (x + 255) / 256 * 256; }
 
@@ -54,6 +56,15 @@ int64_t cw_pool_offset(const cw_config* c, int32_t block, int32_t kv_head, int32
     const int64_t D = c->head_dim;
     return ((int64_t)block * c->num_kv_heads + kv_head) * (CW_BLOCK_SIZE * D) + (t / 8) * (8 * D) + (d / 64) * 512 +
            (t % 8) * 64 + ((((d % 64) / 8) ^ (t % 8)) * 8) + d % 8;
+}
+
+int64_t cw_q_roped_offset(const cw_config* c, int32_t s, int32_t tok, int32_t head, int32_t d) {
+    if (bad_cfg(c) || s <= 0 || tok < 0 || tok >= s || head < 0 || head >= c->num_q_heads || d < 0 || d >= c->head_dim)
+        return CW_ERR_INVALID;
+    const int64_t D = c->head_dim, g = c->num_q_heads / c->num_kv_heads, tpt = 128 / g;
+    const int64_t kvh = head / g, hh = head % g, t = tok / tpt, row = (tok % tpt) * g + hh;
+    const int64_t rows_valid = std::min<int64_t>(tpt, s - t * tpt) * g;
+    return kvh * s * g * D + t * (tpt * g) * D + (d / 64) * rows_valid * 64 + row * 64 + ((((d % 64) / 8) ^ (row % 8)) * 8) + d % 8;
 }
 
 int cw_create(const cw_config* cfg, cw_ctx** out) {
@@ -267,7 +278,7 @@ int cw_gather_kv(cw_ctx* ctx, const int32_t* d_table, int32_t n, void* k_out, vo
 
 int64_t cw_attn_work_ints(cw_ctx* ctx, const int32_t* h_cu, int32_t B) {
     if (!ctx || B < 0 || (B > 0 && !h_cu)) return CW_ERR_INVALID;
-    return 4 * cw::attn_count_tiles(ctx->cfg, h_cu, B);
+    return cw::attn_work_ints(ctx->cfg, h_cu, B);
 }
 
 int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out, const int32_t* h_cu, const int32_t* h_nc,
@@ -291,7 +302,7 @@ int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out, const int32_t* 
     cudaError_t e = cudaMemcpyAsync(d_work, work.data(), work.size() * sizeof(int32_t), cudaMemcpyHostToDevice,
                                     static_cast<cudaStream_t>(stream));   // pageable source: staged before return
     if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_attn (schedule copy)");
-    int le = cw::launch_prefill_attn(ctx->cfg, q_roped, out, d_cu, d_nc, d_tables, max_blocks, d_work, tiles,
+    int le = cw::launch_prefill_attn(ctx->cfg, q_roped, out, d_tables, max_blocks, d_work, tiles,
                                      ctx->num_sms, stream);
     return le ? cuda_fail(ctx, le, "cw_prefill_attn") : CW_OK;
 }
@@ -315,8 +326,9 @@ WsLayout ws_layout(const cw_config& c, int32_t B, int32_t T, int32_t max_blocks)
     w.tables = o; o += align256((int64_t)B * max_blocks * 4);
     // upper bound on tiles: every request may add one ragged tile per kv head
     const int g = c.num_q_heads / c.num_kv_heads;
-    const int64_t max_tiles = (((int64_t)T * g + 127) / 128 + B) * c.num_kv_heads;
-    w.work = o; o += align256(max_tiles * 16);
+    const int tpt2 = 2 * (128 / g);
+    const int64_t max_items = (((int64_t)T + tpt2 - 1) / tpt2 + B) * c.num_kv_heads;
+    w.work = o; o += align256(max_items * 32);
     w.total = o;
     return w;
 }

@@ -60,6 +60,7 @@ __global__ void __launch_bounds__(128) append_kv_kernel(
     const float* __restrict__ rope_table, const int32_t* __restrict__ cu, const int32_t* __restrict__ ncached,
     const int32_t* __restrict__ tables, int max_blocks, int B, int T, int Hq, int Hkv, int max_position) {
     constexpr int CPH = D / 16;                       // chunk pairs (units) per head
+    const int g = Hq / Hkv, tpt = 128 / g;
     const int uq = Hq * CPH, uk = Hkv * CPH;
     const int units = uq + 2 * uk;
     for (int tok = blockIdx.x; tok < T; tok += gridDim.x) {
@@ -70,7 +71,13 @@ __global__ void __launch_bounds__(128) append_kv_kernel(
             if (__ldg(cu + mid) <= tok) lo = mid; else hi = mid;
         }
         const int r = lo;
-        int p = __ldg(ncached + r) + (tok - __ldg(cu + r));
+        const int q_begin = __ldg(cu + r);
+        const int s_len = __ldg(cu + r + 1) - q_begin, tl = tok - q_begin;
+        int p = __ldg(ncached + r) + tl;
+        // q_roped tile: tpt tokens x g heads per (kv head, tile); rows of a tile are stored [64-dim half][row][64], 128B-swizzled
+        const int qt = tl / tpt, tloc = tl - qt * tpt;
+        const int rows_valid = min(tpt, s_len - qt * tpt) * g;
+        const size_t q_tile_base = (size_t)q_begin * Hq * D + (size_t)qt * (tpt * g) * D;
         const int blk = __ldg(tables + (size_t)r * max_blocks + (p >> 4));
         const int tib = p & 15;
         const int prow = p < max_position ? p : max_position - 1;
@@ -81,8 +88,11 @@ __global__ void __launch_bounds__(128) append_kv_kernel(
                 const size_t off = ((size_t)tok * Hq + h) * D + c * 8;
                 uint4 a = ld_stream(q + off), b = ld_stream(q + off + D / 2);
                 rope_pair(a, b, cs_row + c * 4);
-                st_stream(q_roped + off, a);
-                st_stream(q_roped + off + D / 2, b);
+                const int kvh = h / g, row = tloc * g + (h - kvh * g);
+                __nv_bfloat16* qb = q_roped + q_tile_base + (size_t)kvh * s_len * g * D + row * 64;
+                const int d0 = c * 8, d1 = c * 8 + D / 2;
+                st_stream(qb + (d0 >> 6) * rows_valid * 64 + ((((d0 & 63) >> 3) ^ (row & 7)) << 3), a);
+                st_stream(qb + (d1 >> 6) * rows_valid * 64 + ((((d1 & 63) >> 3) ^ (row & 7)) << 3), b);
             } else if (u < uq + uk) {
                 const int uu = u - uq, h = uu / CPH, c = uu % CPH;
                 const size_t off = ((size_t)tok * Hkv + h) * D + c * 8;

@@ -106,11 +106,11 @@ int launch_append_kv(const cw_config& cfg, const void* q, const void* k, const v
                      const int32_t* cu, const int32_t* ncached, const int32_t* tables, int32_t max_blocks,
                      int32_t B, int32_t T, void* stream);
 int launch_gather_kv(const cw_config& cfg, const int32_t* table, int32_t n, void* k_out, void* v_out, void* stream);
-// tile schedule: 4 ints per tile {request, kv_head, first packed row, num kv tokens}; returns tile count
+// attention item list: 8 ints per item (prefill_attn.cu); returns item count
 int64_t attn_count_tiles(const cw_config& cfg, const int32_t* h_cu, int32_t B);
+int64_t attn_work_ints(const cw_config& cfg, const int32_t* h_cu, int32_t B);
 int64_t attn_build_schedule(const cw_config& cfg, const int32_t* h_cu, const int32_t* h_nc, int32_t B,
                             std::vector<int32_t>& work);
-int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* cu,
-                        const int32_t* ncached, const int32_t* tables, int32_t max_blocks, const int32_t* d_work,
-                        int64_t num_tiles, int num_sms, void* stream);
+int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* tables, int32_t max_blocks,
+                        const int32_t* d_work, int64_t num_items, int num_sms, void* stream);
 }  // namespace cw

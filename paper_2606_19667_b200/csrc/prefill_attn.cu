@@ -2,18 +2,22 @@
 //
 //   o[row p, head h] = sum_{j<=p} softmax_j(q'_p . k'_j / sqrt(D)) v_j ,  kv head = h / g
 //
-// Work item ("tile") = (request r, kv head, 128 packed rows).  The g query heads that share a KV head are packed
-// into the M dimension: packed row i <-> (suffix token i / g, head kvh*g + i % g), so one K/V tile read feeds all g
-// heads and short suffixes (query-only after a long cache hit) still fill M = 128.
+// Work item = (request r, kv head, 2 consecutive Q tiles).  A Q tile holds tpt = 128/g suffix tokens x the g query
+// heads that share the kv head, packed into the M dimension (row = token*g + head), so one K/V tile read feeds all g
+// heads and both Q tiles (M = 256 per CTA), and a short query-only suffix still fills the MMA.
 //
-// CTA = 192 threads, warp-specialised, mbarrier pipelines only (no __syncthreads in the main loop):
-//   warps 0-3  softmax / correction / epilogue: thread i owns TMEM lane i = packed row i
-//   warp  4    loader: one bulk copy (UBLKCP) per 16-token pool block per operand, gathered through the block table;
-//              pool blocks are stored pre-swizzled in the UMMA canonical layout (cw_pool_offset), so no re-layout
-//   warp  5    MMA issuer: S = Q K^T (SS, K-major/K-major) into a double-buffered S in TMEM, O += P V (A = P from
-//              smem K-major, B = V MN-major), accumulators in TMEM; also owns TMEM alloc/dealloc
-// Softmax is online in fp32 with exp2 and a lazy rescale: O/l are only rescaled when the running max grows by
-// more than 2^8 (exact: the final normalisation uses the same reference max for O and l).
+// Persistent CTAs (one per SM, 320 threads), static round-robin over a host-built item list, warp-specialised,
+// mbarrier pipelines only:
+//   warps 0-3  softmax / rescale / epilogue of Q tile 0 (thread i owns TMEM lane i = packed row i)
+//   warps 4-7  the same for Q tile 1 — the two groups ping-pong: while one does exp on S_w, the tensor core runs the
+//              other tile's PV and next QK^T
+//   warp  8    MMA issuer: S_w = Q_w K^T (SS) and O_w += P_w V (TS: P is read from TMEM, where the softmax group wrote
+//              it as bf16 over the first half of S_w); owns TMEM alloc/dealloc (512 columns: S0 S1 O0 O1)
+//   warp  9    loader: Q tiles (q_roped is stored tile-packed and pre-swizzled by cw_append_kv: one bulk copy per
+//              64-dim half tile) and K/V tiles (one bulk copy per 16-token pool block per operand, gathered through
+//              the block table; pool blocks are pre-swizzled in the UMMA canonical layout) into a multi-stage ring
+// Softmax is online in fp32 with exp2 and a lazy rescale: O/l are only rescaled when the running max grows by more
+// than 2^8 (exact: the final normalisation uses the same reference max for O and l).
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
@@ -26,28 +30,36 @@ namespace cw {
 
 namespace {
 
-constexpr int kTileM = 128;          // packed query rows per tile
+constexpr int kTileM = 128;          // MMA M (TMEM lanes); a Q tile uses the first tpt*g of them
 constexpr int kTileN = 128;          // keys per KV tile (8 pool blocks)
-constexpr int kStages = 2;           // K and V ring depth
-constexpr int kThreads = 192;
+constexpr int kThreads = 320;
+constexpr int kWorkInts = 8;         // ints per work item
 constexpr float kRescaleThreshold = 8.0f;   // log2 units
 
 template <int D>
 struct Smem {
-    static constexpr int kQBytes = kTileM * D * 2;
-    static constexpr int kKVBytes = kTileN * D * 2;          // one K or V tile
-    static constexpr int kPBytes = kTileM * kTileN * 2;
+    static constexpr int kQBytes = kTileM * D * 2;            // one Q tile
+    static constexpr int kKVBytes = kTileN * D * 2;           // one K or V tile
+    static constexpr int kStages = D == 128 ? 5 : 8;          // K/V ring slots (a K tile or a V tile each)
     static constexpr int kQ = 0;
-    static constexpr int kK = kQ + kQBytes;
-    static constexpr int kV = kK + kStages * kKVBytes;
-    static constexpr int kP = kV + kStages * kKVBytes;
-    static constexpr int kBar = kP + kPBytes;                 // mbarriers (8 B each)
+    static constexpr int kRing = kQ + 2 * kQBytes;
+    static constexpr int kBar = kRing + kStages * kKVBytes;   // mbarriers (8 B each)
     static constexpr int kTotal = kBar + 256;
 };
 
-// barrier slots
-enum { BAR_Q_FULL = 0, BAR_K_FULL = 1, BAR_K_EMPTY = 3, BAR_V_FULL = 5, BAR_V_EMPTY = 7, BAR_S_FULL = 9,
-       BAR_S_EMPTY = 11, BAR_P_FULL = 13, BAR_PV_DONE = 14, BAR_COUNT = 15 };
+// barrier slots (ring FULL[s] at BAR_RING + s, EMPTY[s] at BAR_RING + kStages + s)
+enum { BAR_Q_FULL = 0, BAR_Q_EMPTY = 1, BAR_S_FULL = 2, BAR_P_FULL = 4, BAR_PV_DONE = 6, BAR_O_EMPTY = 8, BAR_RING = 10 };
+
+struct Item {
+    int r, kvh, tok0, pos0, ntok0, ntok1, q_off16;   // q_off16: offset of Q tile 0 inside q_roped in 16-byte units
+};
+
+__device__ __forceinline__ Item load_item(const int4* __restrict__ work, int idx) {
+    const int4 a = __ldg(work + 2 * idx), b = __ldg(work + 2 * idx + 1);
+    return Item{a.x, a.y, a.z, a.w, b.x, b.y, b.z};
+}
+
+__device__ __forceinline__ int tiles_for(int nkv) { return (nkv + kTileN - 1) / kTileN; }
 
 }  // namespace
 
@@ -55,307 +67,355 @@ template <int D>
 __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
     const __nv_bfloat16* __restrict__ q_roped, __nv_bfloat16* __restrict__ out,
     const __nv_bfloat16* __restrict__ k_pool, const __nv_bfloat16* __restrict__ v_pool,
-    const int32_t* __restrict__ cu, const int32_t* __restrict__ ncached, const int32_t* __restrict__ tables,
-    int max_blocks, const int4* __restrict__ work, int Hq, int Hkv, float scale_log2) {
+    const int32_t* __restrict__ tables, int max_blocks, const int4* __restrict__ work, int num_items,
+    int Hq, int Hkv, float scale_log2) {
     using L = Smem<D>;
+    constexpr int NS = L::kStages;
     extern __shared__ __align__(1024) uint8_t smem[];
     const uint32_t sbase = ptx::smem_u32(smem);
     const uint32_t bars = sbase + L::kBar;
     auto bar = [&](int i) { return bars + 8u * (uint32_t)i; };
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kBar + 8 * BAR_COUNT);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(smem + L::kBar + 8 * (BAR_RING + 2 * NS));
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int4 w = __ldg(work + blockIdx.x);
-    const int r = w.x, kvh = w.y, row0 = w.z, num_kv = w.w;
     const int g = Hq / Hkv;
-    const int q_begin = __ldg(cu + r);
-    const int s_len = __ldg(cu + r + 1) - q_begin;
-    const int c = __ldg(ncached + r);
-    const int rows_total = s_len * g;
-    const int n_tiles = (num_kv + kTileN - 1) / kTileN;
+    const int tpt = kTileM / g;          // tokens per Q tile
+    const int R = tpt * g;               // rows of a full Q tile
 
     if (threadIdx.x == 0) {
-        ptx::mbar_init(bar(BAR_Q_FULL), 128);
-        for (int i = 0; i < kStages; ++i) {
-            ptx::mbar_init(bar(BAR_K_FULL + i), 1);
-            ptx::mbar_init(bar(BAR_K_EMPTY + i), 1);
-            ptx::mbar_init(bar(BAR_V_FULL + i), 1);
-            ptx::mbar_init(bar(BAR_V_EMPTY + i), 1);
+        ptx::mbar_init(bar(BAR_Q_FULL), 1);
+        ptx::mbar_init(bar(BAR_Q_EMPTY), 1);
+        for (int w = 0; w < 2; ++w) {
+            ptx::mbar_init(bar(BAR_S_FULL + w), 1);
+            ptx::mbar_init(bar(BAR_P_FULL + w), 128);
+            ptx::mbar_init(bar(BAR_PV_DONE + w), 1);
+            ptx::mbar_init(bar(BAR_O_EMPTY + w), 128);
         }
-        for (int i = 0; i < 2; ++i) {
-            ptx::mbar_init(bar(BAR_S_FULL + i), 1);
-            ptx::mbar_init(bar(BAR_S_EMPTY + i), 128);
-        }
-        ptx::mbar_init(bar(BAR_P_FULL), 128);
-        ptx::mbar_init(bar(BAR_PV_DONE), 1);
+        for (int s = 0; s < 2 * NS; ++s) ptx::mbar_init(bar(BAR_RING + s), 1);
         ptx::fence_mbar_init();
     }
-    if (warp == 5) ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
+    if (warp == 8) ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
-    const uint32_t tmem_S0 = tmem, tmem_O = tmem + 256;
 
-    if (warp == 4) {
+    if (warp == 9) {
         // ================================ loader ================================
         constexpr uint32_t kBlockBytes = 16 * D * 2;
-        const int32_t* table = tables + (size_t)r * max_blocks;
-        for (int j = 0; j < n_tiles; ++j) {
-            const int st = j % kStages;
-            const uint32_t ph = (uint32_t)(j / kStages) & 1u;
-            const int kv_left = num_kv - j * kTileN;
-            const int nblk = kv_left >= kTileN ? 8 : (kv_left + 15) >> 4;
-            int blk = 0;
-            if (lane < nblk) blk = __ldg(table + j * 8 + lane);
-            const size_t src_off = ((size_t)blk * Hkv + kvh) * (16 * D);
-            // K tile
-            ptx::mbar_wait(bar(BAR_K_EMPTY + st), ph ^ 1u);
-            if (lane == 0) ptx::mbar_arrive_expect_tx(bar(BAR_K_FULL + st), kBlockBytes * (uint32_t)nblk);
-            __syncwarp();
-            if (lane < nblk)
-                ptx::bulk_g2s(sbase + L::kK + st * L::kKVBytes + lane * kBlockBytes, k_pool + src_off, kBlockBytes,
-                              bar(BAR_K_FULL + st));
-            // V tile
-            ptx::mbar_wait(bar(BAR_V_EMPTY + st), ph ^ 1u);
-            if (lane == 0) ptx::mbar_arrive_expect_tx(bar(BAR_V_FULL + st), kBlockBytes * (uint32_t)nblk);
-            __syncwarp();
-            if (lane < nblk)
-                ptx::bulk_g2s(sbase + L::kV + st * L::kKVBytes + lane * kBlockBytes, v_pool + src_off, kBlockBytes,
-                              bar(BAR_V_FULL + st));
+        uint32_t it = 0;
+        int item_n = 0;
+        for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x, ++item_n) {
+            const Item w = load_item(work, idx);
+            const int rows0 = w.ntok0 * g, rows1 = w.ntok1 * g;
+            ptx::mbar_wait(bar(BAR_Q_EMPTY), ((uint32_t)item_n & 1u) ^ 1u);
+            if (lane == 0) {
+                ptx::mbar_arrive_expect_tx(bar(BAR_Q_FULL), (uint32_t)((rows0 + rows1) * D * 2));
+                const char* src = reinterpret_cast<const char*>(q_roped) + (size_t)w.q_off16 * 16;
+#pragma unroll
+                for (int h = 0; h < D / 64; ++h)
+                    ptx::bulk_g2s(sbase + L::kQ + h * (kTileM * 128), src + (size_t)h * rows0 * 128, (uint32_t)rows0 * 128u,
+                                  bar(BAR_Q_FULL));
+                if (rows1) {
+                    const char* src1 = src + (size_t)R * D * 2;      // tile 0 is full whenever tile 1 exists
+#pragma unroll
+                    for (int h = 0; h < D / 64; ++h)
+                        ptx::bulk_g2s(sbase + L::kQ + L::kQBytes + h * (kTileM * 128), src1 + (size_t)h * rows1 * 128,
+                                      (uint32_t)rows1 * 128u, bar(BAR_Q_FULL));
+                }
+            }
+            const int nkv = w.pos0 + w.ntok0 + w.ntok1;
+            const int nt = tiles_for(nkv);
+            const int32_t* table = tables + (size_t)w.r * max_blocks;
+            auto load_ids = [&](int j) {
+                const int left = nkv - j * kTileN;
+                const int nb = left >= kTileN ? 8 : (left + 15) >> 4;
+                return lane < nb ? __ldg(table + j * 8 + lane) : 0;
+            };
+            int blk = load_ids(0);
+            for (int j = 0; j < nt; ++j) {
+                const int blk_next = j + 1 < nt ? load_ids(j + 1) : 0;
+                const int left = nkv - j * kTileN;
+                const int nblk = left >= kTileN ? 8 : (left + 15) >> 4;
+                const size_t src_off = ((size_t)blk * Hkv + w.kvh) * (16 * D);
+#pragma unroll
+                for (int kv = 0; kv < 2; ++kv) {
+                    const uint32_t s = it % NS, ph = (it / NS) & 1u;
+                    ptx::mbar_wait(bar(BAR_RING + NS + s), ph ^ 1u);
+                    if (lane == 0) ptx::mbar_arrive_expect_tx(bar(BAR_RING + s), kBlockBytes * (uint32_t)nblk);
+                    __syncwarp();
+                    if (lane < nblk)
+                        ptx::bulk_g2s(sbase + L::kRing + s * L::kKVBytes + lane * kBlockBytes,
+                                      (kv == 0 ? k_pool : v_pool) + src_off, kBlockBytes, bar(BAR_RING + s));
+                    ++it;
+                }
+                blk = blk_next;
+            }
         }
-    } else if (warp == 5) {
-        // ================================ MMA issuer ================================
-        constexpr uint32_t kIdescQK = ptx::umma_idesc_bf16(kTileM, kTileN, 0, 0);
-        constexpr uint32_t kIdescPV = ptx::umma_idesc_bf16(kTileM, D, 0, 1);
-        constexpr uint32_t kGroupStride = (D / 64) * 1024;        // bytes between 8-key groups of a K/V tile
-        auto issue_qk = [&](int j) {
-            const int st = j % kStages;
-            ptx::mbar_wait(bar(BAR_K_FULL + st), (uint32_t)(j / kStages) & 1u);
-            ptx::mbar_wait(bar(BAR_S_EMPTY + (j & 1)), ((uint32_t)(j >> 1) & 1u) ^ 1u);
-            ptx::tc_fence_after();
-            if (ptx::elect_one()) {
-                const uint32_t kb = sbase + L::kK + st * L::kKVBytes;
+    } else if (warp == 8) {
+        // ================================ MMA issuer (one thread) ================================
+        if (lane == 0) {
+            constexpr uint32_t kIdescQK = ptx::umma_idesc_bf16(kTileM, kTileN, 0, 0);
+            constexpr uint32_t kIdescPV = ptx::umma_idesc_bf16(kTileM, D, 0, 1);
+            constexpr uint32_t kGroupStride = (D / 64) * 1024;        // bytes between 8-key groups of a K/V tile
+            uint32_t it = 0, cnt[2] = {0, 0}, oitem[2] = {0, 0};
+            int item_n = 0;
+            auto issue_qk = [&](int w, uint32_t slot) {
+                const uint32_t qb = sbase + L::kQ + w * L::kQBytes, kb = sbase + L::kRing + slot * L::kKVBytes;
 #pragma unroll
                 for (int ks = 0; ks < D / 16; ++ks) {
-                    const uint64_t a = ptx::umma_desc_sw128(sbase + L::kQ + (ks >> 2) * (kTileM * 128) + (ks & 3) * 32, 16, 1024);
+                    const uint64_t a = ptx::umma_desc_sw128(qb + (ks >> 2) * (kTileM * 128) + (ks & 3) * 32, 16, 1024);
                     const uint64_t b = ptx::umma_desc_sw128(kb + (ks >> 2) * 1024 + (ks & 3) * 32, 16, kGroupStride);
-                    ptx::umma_ss(tmem_S0 + (uint32_t)(j & 1) * 128u, a, b, kIdescQK, ks > 0);
+                    ptx::umma_ss(tmem + (uint32_t)w * 128u, a, b, kIdescQK, ks > 0);
                 }
-                ptx::umma_commit(bar(BAR_K_EMPTY + st));
-                ptx::umma_commit(bar(BAR_S_FULL + (j & 1)));
-            }
-            __syncwarp();
-        };
-        ptx::mbar_wait(bar(BAR_Q_FULL), 0);
-        issue_qk(0);
-        for (int j = 0; j < n_tiles; ++j) {
-            if (j + 1 < n_tiles) issue_qk(j + 1);
-            const int st = j % kStages;
-            const int kv_left = num_kv - j * kTileN;
-            const int ksteps = kv_left >= kTileN ? 8 : (kv_left + 15) >> 4;   // skip 16-key steps with no valid key
-            ptx::mbar_wait(bar(BAR_V_FULL + st), (uint32_t)(j / kStages) & 1u);
-            ptx::mbar_wait(bar(BAR_P_FULL), (uint32_t)j & 1u);
-            ptx::tc_fence_after();
-            if (ptx::elect_one()) {
-                const uint32_t vb = sbase + L::kV + st * L::kKVBytes;
-                for (int ks = 0; ks < ksteps; ++ks) {
-                    const uint64_t a = ptx::umma_desc_sw128(sbase + L::kP + (ks >> 2) * (kTileM * 128) + (ks & 3) * 32, 16, 1024);
-                    const uint64_t b = ptx::umma_desc_sw128(vb + ks * 2 * kGroupStride, 1024, kGroupStride);
-                    ptx::umma_ss(tmem_O, a, b, kIdescPV, (j > 0 || ks > 0) ? 1u : 0u);
-                }
-                ptx::umma_commit(bar(BAR_V_EMPTY + st));
-                ptx::umma_commit(bar(BAR_PV_DONE));
-            }
-            __syncwarp();
-        }
-    } else {
-        // ================================ softmax / correction / epilogue ================================
-        const int row = threadIdx.x;                       // TMEM lane == packed row within the tile
-        const int prow = row0 + row;
-        const bool row_valid = prow < rows_total;
-        const int tok = (row_valid ? prow : rows_total - 1) / g;
-        const int hh = (row_valid ? prow : rows_total - 1) % g;
-        const int limit = c + tok;                         // last visible key (inclusive)
-        const uint32_t lane_base = ((uint32_t)(warp * 32)) << 16;
-
-        // ---- Q tile -> smem (K-major, 128B swizzle), zero-filled past the end of the request ----
-        {
-            constexpr int CH = D / 8;                      // 16-byte chunks per row
-            const int ch = threadIdx.x % CH;
-            const __nv_bfloat16* qbase = q_roped + ((size_t)q_begin * Hq + (size_t)kvh * g) * D;
-            for (int rr = threadIdx.x / CH; rr < kTileM; rr += 128 / CH) {
-                const int pr = row0 + rr;
-                uint4 val = make_uint4(0, 0, 0, 0);
-                if (pr < rows_total)
-                    val = *reinterpret_cast<const uint4*>(qbase + ((size_t)(pr / g) * Hq + (pr % g)) * D + ch * 8);
-                const uint32_t dst = sbase + L::kQ + (ch >> 3) * (kTileM * 128) + rr * 128 + (((ch & 7) ^ (rr & 7)) << 4);
-                ptx::st_shared_v4(dst, val.x, val.y, val.z, val.w);
-            }
-            ptx::fence_proxy_async_smem();
-            ptx::mbar_arrive(bar(BAR_Q_FULL));
-        }
-
-        float m_ref = -INFINITY, l_sum = 0.f;
-        for (int j = 0; j < n_tiles; ++j) {
-            const uint32_t tS = tmem_S0 + (uint32_t)(j & 1) * 128u + lane_base;
-            ptx::mbar_wait(bar(BAR_S_FULL + (j & 1)), (uint32_t)(j >> 1) & 1u);
-            ptx::tc_fence_after();
-            uint32_t sv[4][32];
+                ptx::umma_commit(bar(BAR_S_FULL + w));
+            };
+            for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x, ++item_n) {
+                const Item w = load_item(work, idx);
+                const int nkv0 = w.pos0 + w.ntok0, nkv1 = nkv0 + w.ntok1;
+                const int n[2] = {tiles_for(nkv0), w.ntok1 ? tiles_for(nkv1) : 0};
+                const int nt = n[1] ? n[1] : n[0];
+                const int nkv = w.ntok1 ? nkv1 : nkv0;
+                auto slot_of = [&](uint32_t i) { return i % NS; };
+                auto wait_full = [&](uint32_t i) { ptx::mbar_wait(bar(BAR_RING + slot_of(i)), (i / NS) & 1u); };
+                auto release = [&](uint32_t i) { ptx::umma_commit(bar(BAR_RING + NS + slot_of(i))); };
+                ptx::mbar_wait(bar(BAR_Q_FULL), (uint32_t)item_n & 1u);
+                wait_full(it);
+                ptx::tc_fence_after();
+                issue_qk(0, slot_of(it));
+                if (n[1]) issue_qk(1, slot_of(it));
+                release(it);
+                if (nt == 1) ptx::umma_commit(bar(BAR_Q_EMPTY));
+                for (int j = 0; j < nt; ++j) {
+                    const uint32_t iv = it + 2 * j + 1, ikn = it + 2 * j + 2;
+                    const int left = nkv - j * kTileN;
+                    const int ksteps = left >= kTileN ? 8 : (left + 15) >> 4;   // skip 16-key steps with no valid key
+                    wait_full(iv);
+                    bool k_ready = false;
 #pragma unroll
-            for (int i = 0; i < 4; ++i) ptx::tmem_ld32(tS + i * 32, sv[i]);
-            ptx::tmem_ld_wait();
-            ptx::tc_fence_before();
-            ptx::mbar_arrive(bar(BAR_S_EMPTY + (j & 1)));
+                    for (int w2 = 0; w2 < 2; ++w2) {
+                        if (j < n[w2]) {
+                            ptx::mbar_wait(bar(BAR_P_FULL + w2), cnt[w2] & 1u);
+                            if (j == 0) ptx::mbar_wait(bar(BAR_O_EMPTY + w2), (oitem[w2] & 1u) ^ 1u);
+                            ptx::tc_fence_after();
+                            const uint32_t vb = sbase + L::kRing + slot_of(iv) * L::kKVBytes;
+                            for (int ks = 0; ks < ksteps; ++ks) {
+                                const uint64_t b = ptx::umma_desc_sw128(vb + ks * 2 * kGroupStride, 1024, kGroupStride);
+                                ptx::umma_ts(tmem + 256u + (uint32_t)w2 * 128u, tmem + (uint32_t)w2 * 128u + (uint32_t)ks * 8u, b,
+                                             kIdescPV, (j > 0 || ks > 0) ? 1u : 0u);
+                            }
+                            ptx::umma_commit(bar(BAR_PV_DONE + w2));
+                            ++cnt[w2];
+                        }
+                        if (j + 1 < n[w2]) {
+                            if (!k_ready) {
+                                wait_full(ikn);
+                                ptx::tc_fence_after();
+                                k_ready = true;
+                            }
+                            issue_qk(w2, slot_of(ikn));
+                        }
+                    }
+                    release(iv);
+                    if (j + 1 < nt) {
+                        release(ikn);
+                        if (j + 2 == nt) ptx::umma_commit(bar(BAR_Q_EMPTY));
+                    }
+                }
+                it += 2u * (uint32_t)nt;
+                oitem[0] += 1;
+                oitem[1] += n[1] ? 1u : 0u;
+            }
+        }
+        __syncwarp();
+    } else {
+        // ================================ softmax / rescale / epilogue (warps 0-7) ================================
+        const int wg = warp >> 2;                          // Q tile of this group
+        const int row = threadIdx.x & 127;                 // TMEM lane == packed row within the tile
+        const uint32_t lane_base = ((uint32_t)((warp & 3) * 32)) << 16;
+        const uint32_t tS = tmem + (uint32_t)wg * 128u + lane_base;
+        const uint32_t tO = tmem + 256u + (uint32_t)wg * 128u + lane_base;
+        uint32_t cnt = 0;
+        for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
+            const Item w = load_item(work, idx);
+            const int ntok = wg ? w.ntok1 : w.ntok0;
+            if (ntok == 0) continue;
+            const int rows = ntok * g;
+            const bool row_valid = row < rows;
+            const int rr = row_valid ? row : rows - 1;
+            const int tl = wg * tpt + rr / g, hh = rr % g;      // token inside the item, head inside the group
+            const int limit = w.pos0 + tl;                       // last visible key (inclusive)
+            const int n_tiles = tiles_for(w.pos0 + wg * tpt + ntok);
 
-            const int kbase = j * kTileN;
-            if (kbase + kTileN - 1 > limit) {
+            float m_ref = -INFINITY, l_sum = 0.f;
+            for (int j = 0; j < n_tiles; ++j, ++cnt) {
+                ptx::mbar_wait(bar(BAR_S_FULL + wg), cnt & 1u);
+                ptx::tc_fence_after();
+                uint32_t sv[4][32];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) ptx::tmem_ld32(tS + i * 32, sv[i]);
+                ptx::tmem_ld_wait();
+
+                const int kbase = j * kTileN;
+                if (kbase + kTileN - 1 > limit) {
+#pragma unroll
+                    for (int i = 0; i < 4; ++i)
+#pragma unroll
+                        for (int e = 0; e < 32; ++e)
+                            if (kbase + i * 32 + e > limit) sv[i][e] = 0xFF800000u;   // -inf
+                }
+                float tm[4];
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    float a = fmaxf(__uint_as_float(sv[i][0]), __uint_as_float(sv[i][1]));
+                    float b = fmaxf(__uint_as_float(sv[i][2]), __uint_as_float(sv[i][3]));
+#pragma unroll
+                    for (int e = 4; e < 32; e += 4) {
+                        a = fmaxf(a, fmaxf(__uint_as_float(sv[i][e]), __uint_as_float(sv[i][e + 1])));
+                        b = fmaxf(b, fmaxf(__uint_as_float(sv[i][e + 2]), __uint_as_float(sv[i][e + 3])));
+                    }
+                    tm[i] = fmaxf(a, b);
+                }
+                const float tmax = fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3]));
+                // lazy rescale decision (per row); the TMEM round trip below is made warp-uniform
+                float alpha = 1.f;
+                const bool grow = (tmax - m_ref) * scale_log2 > kRescaleThreshold;   // true on the first tile (m_ref = -inf)
+                if (grow) {
+                    alpha = ptx::ex2((m_ref - tmax) * scale_log2);                   // 0 on the first tile
+                    m_ref = tmax;
+                }
+                const float mneg = -m_ref * scale_log2;
+                float ps[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
                 for (int i = 0; i < 4; ++i)
 #pragma unroll
-                    for (int e = 0; e < 32; ++e)
-                        if (kbase + i * 32 + e > limit) sv[i][e] = 0xFF800000u;   // -inf
-            }
-            float tmax = -INFINITY;
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int e = 0; e < 32; ++e) tmax = fmaxf(tmax, __uint_as_float(sv[i][e]));
-            // lazy rescale decision (per row), then made warp-uniform for the TMEM round trip
-            float alpha = 1.f;
-            bool grow = (tmax - m_ref) * scale_log2 > kRescaleThreshold;   // true on the first tile (m_ref = -inf)
-            if (grow) {
-                alpha = ptx::ex2((m_ref - tmax) * scale_log2);             // 0 on the first tile
-                m_ref = tmax;
-            }
-            const float mneg = -m_ref * scale_log2;
-            float psum = 0.f;
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int e = 0; e < 32; e += 2) {
-                    float p0 = ptx::ex2(fmaf(__uint_as_float(sv[i][e]), scale_log2, mneg));
-                    float p1 = ptx::ex2(fmaf(__uint_as_float(sv[i][e + 1]), scale_log2, mneg));
-                    psum += p0 + p1;
-                    sv[i][e >> 1] = ptx::pack_bf16x2(p0, p1);              // packed P overwrites the front half
-                }
-            l_sum = l_sum * alpha + psum;
+                    for (int e = 0; e < 32; e += 2) {
+                        const float p0 = ptx::ex2(fmaf(__uint_as_float(sv[i][e]), scale_log2, mneg));
+                        const float p1 = ptx::ex2(fmaf(__uint_as_float(sv[i][e + 1]), scale_log2, mneg));
+                        ps[(e >> 1) & 3] += p0 + p1;
+                        sv[i >> 1][(i & 1) * 16 + (e >> 1)] = ptx::pack_bf16x2(p0, p1);   // packed P: 64 registers
+                    }
+                l_sum = l_sum * alpha + ((ps[0] + ps[1]) + (ps[2] + ps[3]));
 
-            // P smem and O are free once PV(j-1) has completed
-            if (j > 0) {
-                ptx::mbar_wait(bar(BAR_PV_DONE), (uint32_t)(j - 1) & 1u);
-                ptx::tc_fence_after();
-                if (__any_sync(0xffffffffu, grow)) {
+                if (j > 0 && __any_sync(0xffffffffu, grow)) {
+                    // O_w holds the sum up to tile j-1: S_FULL(j) was committed after PV(j-1), so it is complete
+                    ptx::mbar_wait(bar(BAR_PV_DONE + wg), (cnt - 1u) & 1u);
+                    ptx::tc_fence_after();
 #pragma unroll
                     for (int i = 0; i < D / 32; ++i) {
                         uint32_t o[32];
-                        ptx::tmem_ld32(tmem_O + lane_base + i * 32, o);
+                        ptx::tmem_ld32(tO + i * 32, o);
                         ptx::tmem_ld_wait();
 #pragma unroll
                         for (int e = 0; e < 32; ++e) o[e] = __float_as_uint(__uint_as_float(o[e]) * alpha);
-                        ptx::tmem_st32(tmem_O + lane_base + i * 32, o);
+                        ptx::tmem_st32(tO + i * 32, o);
                     }
-                    ptx::tmem_st_wait();
                 }
+                // P (bf16, two keys per 32-bit column) over the first 64 columns of S_w: A operand of the PV MMA
+                ptx::tmem_st32(tS, sv[0]);
+                ptx::tmem_st32(tS + 32, sv[1]);
+                ptx::tmem_st_wait();
+                ptx::tc_fence_before();
+                ptx::mbar_arrive(bar(BAR_P_FULL + wg));
             }
-            // P (bf16) -> smem, K-major 128B swizzle: [key half][row][64 keys]
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int q4 = 0; q4 < 4; ++q4) {
-                    const int chunk = i * 4 + q4;                           // 8 keys per 16-byte chunk
-                    const uint32_t dst = sbase + L::kP + (chunk >> 3) * (kTileM * 128) + row * 128 +
-                                         (((chunk & 7) ^ (row & 7)) << 4);
-                    ptx::st_shared_v4(dst, sv[i][q4 * 4], sv[i][q4 * 4 + 1], sv[i][q4 * 4 + 2], sv[i][q4 * 4 + 3]);
-                }
-            ptx::fence_proxy_async_smem();
-            ptx::tc_fence_before();
-            ptx::mbar_arrive(bar(BAR_P_FULL));
-        }
 
-        // ---- epilogue: O / l -> bf16 -> global ----
-        ptx::mbar_wait(bar(BAR_PV_DONE), (uint32_t)(n_tiles - 1) & 1u);
-        ptx::tc_fence_after();
-        const float inv_l = 1.f / l_sum;
-        __nv_bfloat16* orow = out + ((size_t)(q_begin + tok) * Hq + (size_t)kvh * g + hh) * D;
+            // ---- epilogue: O / l -> bf16 -> global ----
+            ptx::mbar_wait(bar(BAR_PV_DONE + wg), (cnt - 1u) & 1u);
+            ptx::tc_fence_after();
+            const float inv_l = 1.f / l_sum;
+            __nv_bfloat16* orow = out + ((size_t)(w.tok0 + tl) * Hq + (size_t)w.kvh * g + hh) * D;
 #pragma unroll
-        for (int i = 0; i < D / 32; ++i) {
-            uint32_t o[32];
-            ptx::tmem_ld32(tmem_O + lane_base + i * 32, o);
-            ptx::tmem_ld_wait();
-            if (row_valid) {
+            for (int i = 0; i < D / 32; ++i) {
+                uint32_t o[32];
+                ptx::tmem_ld32(tO + i * 32, o);
+                ptx::tmem_ld_wait();
+                if (row_valid) {
 #pragma unroll
-                for (int e = 0; e < 32; e += 8) {
-                    uint4 pk;
-                    pk.x = ptx::pack_bf16x2(__uint_as_float(o[e]) * inv_l, __uint_as_float(o[e + 1]) * inv_l);
-                    pk.y = ptx::pack_bf16x2(__uint_as_float(o[e + 2]) * inv_l, __uint_as_float(o[e + 3]) * inv_l);
-                    pk.z = ptx::pack_bf16x2(__uint_as_float(o[e + 4]) * inv_l, __uint_as_float(o[e + 5]) * inv_l);
-                    pk.w = ptx::pack_bf16x2(__uint_as_float(o[e + 6]) * inv_l, __uint_as_float(o[e + 7]) * inv_l);
-                    *reinterpret_cast<uint4*>(orow + i * 32 + e) = pk;
+                    for (int e = 0; e < 32; e += 8) {
+                        uint4 pk;
+                        pk.x = ptx::pack_bf16x2(__uint_as_float(o[e]) * inv_l, __uint_as_float(o[e + 1]) * inv_l);
+                        pk.y = ptx::pack_bf16x2(__uint_as_float(o[e + 2]) * inv_l, __uint_as_float(o[e + 3]) * inv_l);
+                        pk.z = ptx::pack_bf16x2(__uint_as_float(o[e + 4]) * inv_l, __uint_as_float(o[e + 5]) * inv_l);
+                        pk.w = ptx::pack_bf16x2(__uint_as_float(o[e + 6]) * inv_l, __uint_as_float(o[e + 7]) * inv_l);
+                        *reinterpret_cast<uint4*>(orow + i * 32 + e) = pk;
+                    }
                 }
             }
+            ptx::tc_fence_before();
+            ptx::mbar_arrive(bar(BAR_O_EMPTY + wg));
         }
-        ptx::tc_fence_before();
     }
 
+    ptx::tc_fence_before();
     __syncthreads();
-    if (warp == 5) {
+    if (warp == 8) {
         ptx::tc_fence_after();
         ptx::tmem_dealloc(tmem, 512);
     }
 }
 
-// ---- host side: tile schedule and launch -------------------------------------------------------------------
+// ---- host side: item list and launch ------------------------------------------------------------------------
+// Items per request: ceil(s / (2*tpt)) * Hkv.
 int64_t attn_count_tiles(const cw_config& cfg, const int32_t* h_cu, int32_t B) {
     const int g = cfg.num_q_heads / cfg.num_kv_heads;
+    const int tpt = kTileM / g;
     int64_t n = 0;
     for (int r = 0; r < B; ++r) {
-        int64_t rows = (int64_t)(h_cu[r + 1] - h_cu[r]) * g;
-        n += (rows + kTileM - 1) / kTileM * cfg.num_kv_heads;
+        const int64_t s = h_cu[r + 1] - h_cu[r];
+        n += (s + 2 * tpt - 1) / (2 * tpt) * cfg.num_kv_heads;
     }
     return n;
 }
 
-// Longest-first order: CTAs are dispatched in blockIdx order, so sorting tiles by descending KV length gives an
-// LPT schedule over the 148 SMs without a persistent loop.
-int64_t attn_build_schedule(const cw_config& cfg, const int32_t* h_cu, const int32_t* h_nc, int32_t B,
-                            std::vector<int32_t>& work) {
-    const int g = cfg.num_q_heads / cfg.num_kv_heads;
-    struct T { int32_t r, kvh, row0, nkv; };
-    std::vector<T> tiles;
-    for (int r = 0; r < B; ++r) {
-        const int s = h_cu[r + 1] - h_cu[r];
-        const int64_t rows = (int64_t)s * g;
-        for (int64_t row0 = 0; row0 < rows; row0 += kTileM) {
-            const int64_t last = std::min<int64_t>(row0 + kTileM - 1, rows - 1);
-            const int32_t nkv = h_nc[r] + (int32_t)(last / g) + 1;
-            for (int kvh = 0; kvh < cfg.num_kv_heads; ++kvh) tiles.push_back(T{r, kvh, (int32_t)row0, nkv});
-        }
-    }
-    std::stable_sort(tiles.begin(), tiles.end(), [](const T& a, const T& b) { return a.nkv > b.nkv; });
-    work.resize(tiles.size() * 4);
-    for (size_t i = 0; i < tiles.size(); ++i) {
-        work[4 * i] = tiles[i].r; work[4 * i + 1] = tiles[i].kvh; work[4 * i + 2] = tiles[i].row0; work[4 * i + 3] = tiles[i].nkv;
-    }
-    return (int64_t)tiles.size();
+int64_t attn_work_ints(const cw_config& cfg, const int32_t* h_cu, int32_t B) {
+    return kWorkInts * attn_count_tiles(cfg, h_cu, B);
 }
 
-int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* cu,
-                        const int32_t* ncached, const int32_t* tables, int32_t max_blocks, const int32_t* d_work,
-                        int64_t num_tiles, int /*num_sms*/, void* stream) {
-    if (num_tiles == 0) return 0;
+// Item order: requests by descending work (longest first, so the tail of the launch is made of short items); inside
+// a request kv-head major, tile pairs by descending kv length.  CTA b takes items b, b+G, b+2G, ...: the CTAs work
+// on neighbouring items of the same (request, kv head) at the same time and share its K/V blocks through L2.
+int64_t attn_build_schedule(const cw_config& cfg, const int32_t* h_cu, const int32_t* h_nc, int32_t B,
+                            std::vector<int32_t>& work) {
+    const int g = cfg.num_q_heads / cfg.num_kv_heads, D = cfg.head_dim, Hq = cfg.num_q_heads;
+    const int tpt = kTileM / g, R = tpt * g;
+    std::vector<int32_t> reqs((size_t)B);
+    for (int r = 0; r < B; ++r) reqs[(size_t)r] = r;
+    auto work_of = [&](int r) {
+        const int64_t s = h_cu[r + 1] - h_cu[r], c = h_nc[r];
+        return s * (2 * c + s);                      // ~ number of (row, key) pairs
+    };
+    std::stable_sort(reqs.begin(), reqs.end(), [&](int a, int b) { return work_of(a) > work_of(b); });
+    work.clear();
+    for (int r : reqs) {
+        const int s = h_cu[r + 1] - h_cu[r];
+        const int npair = (s + 2 * tpt - 1) / (2 * tpt);
+        for (int kvh = 0; kvh < cfg.num_kv_heads; ++kvh)
+            for (int t = npair - 1; t >= 0; --t) {
+                const int tok0 = t * 2 * tpt;
+                const int ntok0 = std::min(tpt, s - tok0), ntok1 = std::max(0, std::min(tpt, s - tok0 - tpt));
+                const int64_t q_off = ((int64_t)h_cu[r] * Hq + (int64_t)kvh * s * g) * D + (int64_t)t * 2 * R * D;   // elements
+                const int32_t item[kWorkInts] = {r, kvh, h_cu[r] + tok0, h_nc[r] + tok0, ntok0, ntok1, (int32_t)(q_off / 8), 0};
+                work.insert(work.end(), item, item + kWorkInts);
+            }
+    }
+    return (int64_t)work.size() / kWorkInts;
+}
+
+int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* tables, int32_t max_blocks,
+                        const int32_t* d_work, int64_t num_items, int num_sms, void* stream) {
+    if (num_items == 0) return 0;
     auto s = static_cast<cudaStream_t>(stream);
     const float scale_log2 = 1.4426950408889634f / sqrtf((float)cfg.head_dim);
-    // both head dims request the same dynamic smem so that exactly one CTA (512 TMEM columns) is resident per SM
-    const int smem_bytes = Smem<128>::kTotal;
+    const unsigned grid = (unsigned)std::min<int64_t>(num_items, num_sms);
     cudaError_t e;
 #define CW_LAUNCH_ATTN(DD)                                                                                          \
     do {                                                                                                            \
-        e = cudaFuncSetAttribute(prefill_attn_kernel<DD>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes); \
+        e = cudaFuncSetAttribute(prefill_attn_kernel<DD>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
+                                 Smem<DD>::kTotal);                                                                 \
         if (e != cudaSuccess) return (int)e;                                                                        \
-        prefill_attn_kernel<DD><<<(unsigned)num_tiles, kThreads, smem_bytes, s>>>(                                  \
+        prefill_attn_kernel<DD><<<grid, kThreads, Smem<DD>::kTotal, s>>>(                                           \
             (const __nv_bfloat16*)q_roped, (__nv_bfloat16*)out, (const __nv_bfloat16*)cfg.k_pool,                   \
-            (const __nv_bfloat16*)cfg.v_pool, cu, ncached, tables, max_blocks, (const int4*)d_work,                 \
+            (const __nv_bfloat16*)cfg.v_pool, tables, max_blocks, (const int4*)d_work, (int)num_items,              \
             cfg.num_q_heads, cfg.num_kv_heads, scale_log2);                                                         \
     } while (0)
     if (cfg.head_dim == 128) CW_LAUNCH_ATTN(128); else CW_LAUNCH_ATTN(64);

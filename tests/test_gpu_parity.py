@@ -57,6 +57,19 @@ def assert_bf16_ulp(got_bits, ref, what=""):
     assert not bad.any(), f"{what}: {bad.sum()} elements off by more than 1 bf16 ulp (max err {err.max():.3e})"
 
 
+def unpack_q_roped(flat_bits, s, Hq, Hkv, D):
+    """tile-packed q_roped slice of one request (cacheweaver.h: cw_q_roped_offset) -> plain [s, Hq, D]."""
+    g = Hq // Hkv
+    tpt = 128 // g
+    tok, head, d = np.meshgrid(np.arange(s), np.arange(Hq), np.arange(D), indexing="ij")
+    kvh, hh, t = head // g, head % g, tok // tpt
+    row = (tok % tpt) * g + hh
+    rows = np.minimum(tpt, s - t * tpt) * g
+    off = kvh * s * g * D + t * (tpt * g) * D + (d // 64) * rows * 64 + row * 64 + ((((d % 64) // 8) ^ (row % 8)) * 8) + d % 8
+    assert np.array_equal(np.sort(off.ravel()), np.arange(s * Hq * D)), "the layout must be a permutation"
+    return flat_bits.reshape(-1)[off]
+
+
 class Batch:
     """Hand-built varlen batch: request r has n_cached c[r] (multiple of 16) and suffix length s[r]; block tables are
     a seeded permutation of the pool.  The prefix K/V is written by a first cw_append_kv call with c = 0."""
@@ -123,7 +136,11 @@ def test_append_kv_pool_contents_and_q_roped(dev, Hq, Hkv, D):
         pos = np.arange(n)
         k_ref = oattn.rope(f(b.k[r]), pos, b.theta)
         q_ref = oattn.rope(f(b.q[r]), pos, b.theta)[c:]
-        assert_bf16_ulp(qr_bits[cu[r]:cu[r + 1]], q_ref, f"q_roped r={r}")
+        qr = unpack_q_roped(qr_bits[cu[r]:cu[r + 1]], n - c, Hq, Hkv, D)
+        assert_bf16_ulp(qr, q_ref, f"q_roped r={r}")
+        flat = qr_bits[cu[r]:cu[r + 1]].reshape(-1)
+        for (t, h, d) in [(0, 0, 0), (n - c - 1, Hq - 1, D - 1), ((n - c) // 2, Hq // 2, 37)]:
+            assert flat[b.ctx.cw_q_roped_offset(n - c, t, h, d)] == qr[t, h, d]
         k_out = torch.empty(n, Hkv, D, dtype=torch.bfloat16, device=dev)
         v_out = torch.empty_like(k_out)
         d_table = torch.from_numpy(b.tables[r]).to(dev)
@@ -141,7 +158,7 @@ def test_append_kv_pool_contents_and_q_roped(dev, Hq, Hkv, D):
 def test_append_kv_position_zero_is_identity(dev):
     b = Batch(dev, 4, 2, 128, cs=[0], ss=[1], seed=2)
     qr_bits, out_bits, _ = b.run()
-    assert np.array_equal(qr_bits[0], b.q[0][0])            # RoPE at p = 0 is the identity
+    assert np.array_equal(unpack_q_roped(qr_bits, 1, 4, 2, 128)[0], b.q[0][0])   # RoPE at p = 0 is the identity
     # row p = 0 attends only key 0: o = v_0 exactly (bit-exact bf16)
     g = 2
     for h in range(4):
