@@ -6,14 +6,15 @@
 // heads that share the kv head, packed into the M dimension (row = token*g + head), so one K/V tile read feeds all g
 // heads and both Q tiles (M = 256 per CTA), and a short query-only suffix still fills the MMA.
 //
-// Persistent CTAs (one per SM, 320 threads), static round-robin over a host-built item list, warp-specialised,
-// mbarrier pipelines only:
-//   warps 0-3  softmax / rescale / epilogue of Q tile 0 (thread i owns TMEM lane i = packed row i)
-//   warps 4-7  the same for Q tile 1 — the two groups ping-pong: while one does exp on S_w, the tensor core runs the
-//              other tile's PV and next QK^T
-//   warp  8    MMA issuer: S_w = Q_w K^T (SS) and O_w += P_w V (TS: P is read from TMEM, where the softmax group wrote
-//              it as bf16 over the first half of S_w); owns TMEM alloc/dealloc (512 columns: S0 S1 O0 O1)
-//   warp  9    loader: Q tiles (q_roped is stored tile-packed and pre-swizzled by cw_append_kv: one bulk copy per
+// Persistent CTAs (one per SM, 512 threads = 4 warpgroups), static round-robin over a host-built item list,
+// warp-specialised, mbarrier pipelines only; registers are re-balanced with setmaxnreg (softmax 192, epilogue 80, rest 48):
+//   warps 0-3   softmax + lazy rescale of Q tile 0 (thread i owns TMEM lane i = packed row i)
+//   warps 4-7   the same for Q tile 1 — the two groups ping-pong: while one does exp on S_w, the tensor core runs the
+//               other tile's PV and next QK^T
+//   warps 8-11  epilogue of both tiles: O_w / l_w -> bf16 -> global, so the softmax groups go straight on to the next item
+//   warp  12    MMA issuer: S_w = Q_w K^T (SS) and O_w += P_w V (TS: P is read from TMEM, where the softmax group wrote
+//               it as bf16 over the first half of S_w); owns TMEM alloc/dealloc (512 columns: S0 S1 O0 O1)
+//   warp  13    loader: Q tiles (q_roped is stored tile-packed and pre-swizzled by cw_append_kv: one bulk copy per
 //              64-dim half tile) and K/V tiles (one bulk copy per 16-token pool block per operand, gathered through
 //              the block table; pool blocks are pre-swizzled in the UMMA canonical layout) into a multi-stage ring
 // Softmax is online in fp32 with exp2 and a lazy rescale: O/l are only rescaled when the running max grows by more
@@ -32,7 +33,7 @@ namespace {
 
 constexpr int kTileM = 128;          // MMA M (TMEM lanes); a Q tile uses the first tpt*g of them
 constexpr int kTileN = 128;          // keys per KV tile (8 pool blocks)
-constexpr int kThreads = 320;
+constexpr int kThreads = 512;
 constexpr int kWorkInts = 8;         // ints per work item
 constexpr float kRescaleThreshold = 8.0f;   // log2 units
 
@@ -43,12 +44,14 @@ struct Smem {
     static constexpr int kStages = D == 128 ? 5 : 8;          // K/V ring slots (a K tile or a V tile each)
     static constexpr int kQ = 0;
     static constexpr int kRing = kQ + 2 * kQBytes;
-    static constexpr int kBar = kRing + kStages * kKVBytes;   // mbarriers (8 B each)
-    static constexpr int kTotal = kBar + 256;
+    static constexpr int kBar = kRing + kStages * kKVBytes;   // mbarriers (8 B each), then the TMEM slot
+    static constexpr int kL = kBar + 256;                     // l_sum hand-off softmax -> epilogue: float [2][128]
+    static constexpr int kTotal = kL + 1024;
 };
 
 // barrier slots (ring FULL[s] at BAR_RING + s, EMPTY[s] at BAR_RING + kStages + s)
-enum { BAR_Q_FULL = 0, BAR_Q_EMPTY = 1, BAR_S_FULL = 2, BAR_P_FULL = 4, BAR_PV_DONE = 6, BAR_O_EMPTY = 8, BAR_RING = 10 };
+enum { BAR_Q_FULL = 0, BAR_Q_EMPTY = 1, BAR_S_FULL = 2, BAR_P_FULL = 4, BAR_PV_DONE = 6, BAR_O_EMPTY = 8, BAR_L_FULL = 10,
+       BAR_L_EMPTY = 12, BAR_RING = 14 };
 
 struct Item {
     int r, kvh, tok0, pos0, ntok0, ntok1, q_off16;   // q_off16: offset of Q tile 0 inside q_roped in 16-byte units
@@ -90,75 +93,80 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
             ptx::mbar_init(bar(BAR_P_FULL + w), 128);
             ptx::mbar_init(bar(BAR_PV_DONE + w), 1);
             ptx::mbar_init(bar(BAR_O_EMPTY + w), 128);
+            ptx::mbar_init(bar(BAR_L_FULL + w), 128);
+            ptx::mbar_init(bar(BAR_L_EMPTY + w), 128);
         }
         for (int s = 0; s < 2 * NS; ++s) ptx::mbar_init(bar(BAR_RING + s), 1);
         ptx::fence_mbar_init();
     }
-    if (warp == 8) ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
+    if (warp == 12) ptx::tmem_alloc(ptx::smem_u32(tmem_slot), 512);
     ptx::tc_fence_before();
     __syncthreads();
     ptx::tc_fence_after();
     const uint32_t tmem = *tmem_slot;
 
-    if (warp == 9) {
-        // ================================ loader ================================
-        constexpr uint32_t kBlockBytes = 16 * D * 2;
-        uint32_t it = 0;
-        int item_n = 0;
-        for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x, ++item_n) {
-            const Item w = load_item(work, idx);
-            const int rows0 = w.ntok0 * g, rows1 = w.ntok1 * g;
-            ptx::mbar_wait(bar(BAR_Q_EMPTY), ((uint32_t)item_n & 1u) ^ 1u);
-            if (lane == 0) {
-                ptx::mbar_arrive_expect_tx(bar(BAR_Q_FULL), (uint32_t)((rows0 + rows1) * D * 2));
-                const char* src = reinterpret_cast<const char*>(q_roped) + (size_t)w.q_off16 * 16;
-#pragma unroll
-                for (int h = 0; h < D / 64; ++h)
-                    ptx::bulk_g2s(sbase + L::kQ + h * (kTileM * 128), src + (size_t)h * rows0 * 128, (uint32_t)rows0 * 128u,
-                                  bar(BAR_Q_FULL));
-                if (rows1) {
-                    const char* src1 = src + (size_t)R * D * 2;      // tile 0 is full whenever tile 1 exists
+    if (warp >= 12) {
+        ptx::setmaxnreg_dec<48>();
+        if (warp == 13) {
+            // ================================ loader ================================
+            constexpr uint32_t kBlockBytes = 16 * D * 2;
+            uint32_t it = 0;
+            int item_n = 0;
+            Item nxt = load_item(work, blockIdx.x);
+            for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x, ++item_n) {
+                const Item w = nxt;
+                if (idx + (int)gridDim.x < num_items) nxt = load_item(work, idx + gridDim.x);
+                const int rows0 = w.ntok0 * g, rows1 = w.ntok1 * g;
+                const int nkv = w.pos0 + w.ntok0 + w.ntok1;
+                const int nt = tiles_for(nkv);
+                const int32_t* table = tables + (size_t)w.r * max_blocks;
+                auto load_ids = [&](int j) {
+                    const int left = nkv - j * kTileN;
+                    const int nb = left >= kTileN ? 8 : (left + 15) >> 4;
+                    return lane < nb ? __ldg(table + j * 8 + lane) : 0;
+                };
+                int blk = load_ids(0);
+                ptx::mbar_wait(bar(BAR_Q_EMPTY), ((uint32_t)item_n & 1u) ^ 1u);
+                if (lane == 0) {
+                    ptx::mbar_arrive_expect_tx(bar(BAR_Q_FULL), (uint32_t)((rows0 + rows1) * D * 2));
+                    const char* src = reinterpret_cast<const char*>(q_roped) + (size_t)w.q_off16 * 16;
 #pragma unroll
                     for (int h = 0; h < D / 64; ++h)
-                        ptx::bulk_g2s(sbase + L::kQ + L::kQBytes + h * (kTileM * 128), src1 + (size_t)h * rows1 * 128,
-                                      (uint32_t)rows1 * 128u, bar(BAR_Q_FULL));
-                }
-            }
-            const int nkv = w.pos0 + w.ntok0 + w.ntok1;
-            const int nt = tiles_for(nkv);
-            const int32_t* table = tables + (size_t)w.r * max_blocks;
-            auto load_ids = [&](int j) {
-                const int left = nkv - j * kTileN;
-                const int nb = left >= kTileN ? 8 : (left + 15) >> 4;
-                return lane < nb ? __ldg(table + j * 8 + lane) : 0;
-            };
-            int blk = load_ids(0);
-            for (int j = 0; j < nt; ++j) {
-                const int blk_next = j + 1 < nt ? load_ids(j + 1) : 0;
-                const int left = nkv - j * kTileN;
-                const int nblk = left >= kTileN ? 8 : (left + 15) >> 4;
-                const size_t src_off = ((size_t)blk * Hkv + w.kvh) * (16 * D);
+                        ptx::bulk_g2s(sbase + L::kQ + h * (kTileM * 128), src + (size_t)h * rows0 * 128,
+                                      (uint32_t)rows0 * 128u, bar(BAR_Q_FULL));
+                    if (rows1) {
+                        const char* src1 = src + (size_t)R * D * 2;      // tile 0 is full whenever tile 1 exists
 #pragma unroll
-                for (int kv = 0; kv < 2; ++kv) {
-                    const uint32_t s = it % NS, ph = (it / NS) & 1u;
-                    ptx::mbar_wait(bar(BAR_RING + NS + s), ph ^ 1u);
-                    if (lane == 0) ptx::mbar_arrive_expect_tx(bar(BAR_RING + s), kBlockBytes * (uint32_t)nblk);
-                    __syncwarp();
-                    if (lane < nblk)
-                        ptx::bulk_g2s(sbase + L::kRing + s * L::kKVBytes + lane * kBlockBytes,
-                                      (kv == 0 ? k_pool : v_pool) + src_off, kBlockBytes, bar(BAR_RING + s));
-                    ++it;
+                        for (int h = 0; h < D / 64; ++h)
+                            ptx::bulk_g2s(sbase + L::kQ + L::kQBytes + h * (kTileM * 128), src1 + (size_t)h * rows1 * 128,
+                                          (uint32_t)rows1 * 128u, bar(BAR_Q_FULL));
+                    }
                 }
-                blk = blk_next;
+                for (int j = 0; j < nt; ++j) {
+                    const int blk_next = j + 1 < nt ? load_ids(j + 1) : 0;
+                    const int left = nkv - j * kTileN;
+                    const int nblk = left >= kTileN ? 8 : (left + 15) >> 4;
+                    const size_t src_off = ((size_t)blk * Hkv + w.kvh) * (16 * D);
+#pragma unroll
+                    for (int kv = 0; kv < 2; ++kv) {
+                        const uint32_t s = it % NS, ph = (it / NS) & 1u;
+                        ptx::mbar_wait(bar(BAR_RING + NS + s), ph ^ 1u);
+                        if (lane == 0) ptx::mbar_arrive_expect_tx(bar(BAR_RING + s), kBlockBytes * (uint32_t)nblk);
+                        __syncwarp();
+                        if (lane < nblk)
+                            ptx::bulk_g2s(sbase + L::kRing + s * L::kKVBytes + lane * kBlockBytes,
+                                          (kv == 0 ? k_pool : v_pool) + src_off, kBlockBytes, bar(BAR_RING + s));
+                        ++it;
+                    }
+                    blk = blk_next;
+                }
             }
-        }
-    } else if (warp == 8) {
-        // ================================ MMA issuer (one thread) ================================
-        if (lane == 0) {
+        } else if (warp == 12 && lane == 0) {
+            // ================================ MMA issuer (one thread) ================================
             constexpr uint32_t kIdescQK = ptx::umma_idesc_bf16(kTileM, kTileN, 0, 0);
             constexpr uint32_t kIdescPV = ptx::umma_idesc_bf16(kTileM, D, 0, 1);
             constexpr uint32_t kGroupStride = (D / 64) * 1024;        // bytes between 8-key groups of a K/V tile
-            uint32_t it = 0, cnt[2] = {0, 0}, oitem[2] = {0, 0};
+            uint32_t it = 0, cnt0 = 0, cnt1 = 0, oitem0 = 0, oitem1 = 0;
             int item_n = 0;
             auto issue_qk = [&](int w, uint32_t slot) {
                 const uint32_t qb = sbase + L::kQ + w * L::kQBytes, kb = sbase + L::kRing + slot * L::kKVBytes;
@@ -170,11 +178,22 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 }
                 ptx::umma_commit(bar(BAR_S_FULL + w));
             };
+            auto issue_pv = [&](int w, uint32_t slot, int ksteps, bool first) {
+                const uint32_t vb = sbase + L::kRing + slot * L::kKVBytes;
+                for (int ks = 0; ks < ksteps; ++ks) {
+                    const uint64_t b = ptx::umma_desc_sw128(vb + ks * 2 * kGroupStride, 1024, kGroupStride);
+                    ptx::umma_ts(tmem + 256u + (uint32_t)w * 128u, tmem + (uint32_t)w * 128u + (uint32_t)ks * 8u, b, kIdescPV,
+                                 (!first || ks > 0) ? 1u : 0u);
+                }
+                ptx::umma_commit(bar(BAR_PV_DONE + w));
+            };
+            Item nxt = load_item(work, blockIdx.x);
             for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x, ++item_n) {
-                const Item w = load_item(work, idx);
+                const Item w = nxt;
+                if (idx + (int)gridDim.x < num_items) nxt = load_item(work, idx + gridDim.x);
                 const int nkv0 = w.pos0 + w.ntok0, nkv1 = nkv0 + w.ntok1;
-                const int n[2] = {tiles_for(nkv0), w.ntok1 ? tiles_for(nkv1) : 0};
-                const int nt = n[1] ? n[1] : n[0];
+                const int n0 = tiles_for(nkv0), n1 = w.ntok1 ? tiles_for(nkv1) : 0;
+                const int nt = n1 ? n1 : n0;
                 const int nkv = w.ntok1 ? nkv1 : nkv0;
                 auto slot_of = [&](uint32_t i) { return i % NS; };
                 auto wait_full = [&](uint32_t i) { ptx::mbar_wait(bar(BAR_RING + slot_of(i)), (i / NS) & 1u); };
@@ -183,7 +202,7 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 wait_full(it);
                 ptx::tc_fence_after();
                 issue_qk(0, slot_of(it));
-                if (n[1]) issue_qk(1, slot_of(it));
+                if (n1) issue_qk(1, slot_of(it));
                 release(it);
                 if (nt == 1) ptx::umma_commit(bar(BAR_Q_EMPTY));
                 for (int j = 0; j < nt; ++j) {
@@ -192,29 +211,34 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                     const int ksteps = left >= kTileN ? 8 : (left + 15) >> 4;   // skip 16-key steps with no valid key
                     wait_full(iv);
                     bool k_ready = false;
-#pragma unroll
-                    for (int w2 = 0; w2 < 2; ++w2) {
-                        if (j < n[w2]) {
-                            ptx::mbar_wait(bar(BAR_P_FULL + w2), cnt[w2] & 1u);
-                            if (j == 0) ptx::mbar_wait(bar(BAR_O_EMPTY + w2), (oitem[w2] & 1u) ^ 1u);
+                    // ---- Q tile 0 ----
+                    if (j < n0) {
+                        ptx::mbar_wait(bar(BAR_P_FULL + 0), cnt0 & 1u);
+                        if (j == 0) ptx::mbar_wait(bar(BAR_O_EMPTY + 0), (oitem0 & 1u) ^ 1u);
+                        ptx::tc_fence_after();
+                        issue_pv(0, slot_of(iv), ksteps, j == 0);
+                        ++cnt0;
+                    }
+                    if (j + 1 < n0) {
+                        wait_full(ikn);
+                        ptx::tc_fence_after();
+                        k_ready = true;
+                        issue_qk(0, slot_of(ikn));
+                    }
+                    // ---- Q tile 1 ----
+                    if (j < n1) {
+                        ptx::mbar_wait(bar(BAR_P_FULL + 1), cnt1 & 1u);
+                        if (j == 0) ptx::mbar_wait(bar(BAR_O_EMPTY + 1), (oitem1 & 1u) ^ 1u);
+                        ptx::tc_fence_after();
+                        issue_pv(1, slot_of(iv), ksteps, j == 0);
+                        ++cnt1;
+                    }
+                    if (j + 1 < n1) {
+                        if (!k_ready) {
+                            wait_full(ikn);
                             ptx::tc_fence_after();
-                            const uint32_t vb = sbase + L::kRing + slot_of(iv) * L::kKVBytes;
-                            for (int ks = 0; ks < ksteps; ++ks) {
-                                const uint64_t b = ptx::umma_desc_sw128(vb + ks * 2 * kGroupStride, 1024, kGroupStride);
-                                ptx::umma_ts(tmem + 256u + (uint32_t)w2 * 128u, tmem + (uint32_t)w2 * 128u + (uint32_t)ks * 8u, b,
-                                             kIdescPV, (j > 0 || ks > 0) ? 1u : 0u);
-                            }
-                            ptx::umma_commit(bar(BAR_PV_DONE + w2));
-                            ++cnt[w2];
                         }
-                        if (j + 1 < n[w2]) {
-                            if (!k_ready) {
-                                wait_full(ikn);
-                                ptx::tc_fence_after();
-                                k_ready = true;
-                            }
-                            issue_qk(w2, slot_of(ikn));
-                        }
+                        issue_qk(1, slot_of(ikn));
                     }
                     release(iv);
                     if (j + 1 < nt) {
@@ -223,28 +247,74 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                     }
                 }
                 it += 2u * (uint32_t)nt;
-                oitem[0] += 1;
-                oitem[1] += n[1] ? 1u : 0u;
+                oitem0 += 1;
+                oitem1 += n1 ? 1u : 0u;
             }
         }
         __syncwarp();
+    } else if (warp >= 8) {
+        // ================================ epilogue (warps 8-11): O_w / l_w -> bf16 -> global ================================
+        ptx::setmaxnreg_dec<80>();
+        const int row = threadIdx.x & 127;                 // TMEM lane == packed row within a tile
+        const uint32_t lane_base = ((uint32_t)((warp & 3) * 32)) << 16;
+        const int tdiv = row / g, hh = row - tdiv * g;
+        uint32_t cnt[2] = {0, 0}, litem[2] = {0, 0};
+        Item nxt = load_item(work, blockIdx.x);
+        for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
+            const Item w = nxt;
+            if (idx + (int)gridDim.x < num_items) nxt = load_item(work, idx + gridDim.x);
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                const int ntok = t ? w.ntok1 : w.ntok0;
+                if (ntok == 0) continue;
+                cnt[t] += (uint32_t)tiles_for(w.pos0 + t * tpt + ntok);
+                const bool row_valid = row < ntok * g;
+                ptx::mbar_wait(bar(BAR_L_FULL + t), litem[t] & 1u);
+                const float inv_l = 1.f / ptx::ld_shared_f32(sbase + L::kL + (t * 128 + row) * 4);
+                ptx::mbar_arrive(bar(BAR_L_EMPTY + t));
+                ++litem[t];
+                ptx::mbar_wait(bar(BAR_PV_DONE + t), (cnt[t] - 1u) & 1u);
+                ptx::tc_fence_after();
+                const uint32_t tO = tmem + 256u + (uint32_t)t * 128u + lane_base;
+                __nv_bfloat16* orow = out + ((size_t)(w.tok0 + t * tpt + tdiv) * Hq + (size_t)w.kvh * g + hh) * D;
+#pragma unroll
+                for (int i = 0; i < D / 32; ++i) {
+                    uint32_t o[32];
+                    ptx::tmem_ld32(tO + i * 32, o);
+                    ptx::tmem_ld_wait();
+                    if (row_valid) {
+#pragma unroll
+                        for (int e = 0; e < 32; e += 8) {
+                            uint4 pk;
+                            pk.x = ptx::pack_bf16x2(__uint_as_float(o[e]) * inv_l, __uint_as_float(o[e + 1]) * inv_l);
+                            pk.y = ptx::pack_bf16x2(__uint_as_float(o[e + 2]) * inv_l, __uint_as_float(o[e + 3]) * inv_l);
+                            pk.z = ptx::pack_bf16x2(__uint_as_float(o[e + 4]) * inv_l, __uint_as_float(o[e + 5]) * inv_l);
+                            pk.w = ptx::pack_bf16x2(__uint_as_float(o[e + 6]) * inv_l, __uint_as_float(o[e + 7]) * inv_l);
+                            *reinterpret_cast<uint4*>(orow + i * 32 + e) = pk;
+                        }
+                    }
+                }
+                ptx::tc_fence_before();
+                ptx::mbar_arrive(bar(BAR_O_EMPTY + t));
+            }
+        }
     } else {
-        // ================================ softmax / rescale / epilogue (warps 0-7) ================================
+        // ================================ softmax + lazy rescale (warps 0-7) ================================
+        ptx::setmaxnreg_inc<192>();
         const int wg = warp >> 2;                          // Q tile of this group
         const int row = threadIdx.x & 127;                 // TMEM lane == packed row within the tile
         const uint32_t lane_base = ((uint32_t)((warp & 3) * 32)) << 16;
         const uint32_t tS = tmem + (uint32_t)wg * 128u + lane_base;
         const uint32_t tO = tmem + 256u + (uint32_t)wg * 128u + lane_base;
-        uint32_t cnt = 0;
+        const int tl = wg * tpt + row / g;                 // token of this row inside the item
+        uint32_t cnt = 0, litem = 0;
+        Item nxt = load_item(work, blockIdx.x);
         for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
-            const Item w = load_item(work, idx);
+            const Item w = nxt;
+            if (idx + (int)gridDim.x < num_items) nxt = load_item(work, idx + gridDim.x);
             const int ntok = wg ? w.ntok1 : w.ntok0;
             if (ntok == 0) continue;
-            const int rows = ntok * g;
-            const bool row_valid = row < rows;
-            const int rr = row_valid ? row : rows - 1;
-            const int tl = wg * tpt + rr / g, hh = rr % g;      // token inside the item, head inside the group
-            const int limit = w.pos0 + tl;                       // last visible key (inclusive)
+            const int limit = w.pos0 + tl;                 // last visible key (inclusive); rows past the tile end are never stored
             const int n_tiles = tiles_for(w.pos0 + wg * tpt + ntok);
 
             float m_ref = -INFINITY, l_sum = 0.f;
@@ -285,17 +355,19 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                     m_ref = tmax;
                 }
                 const float mneg = -m_ref * scale_log2;
-                float ps[4] = {0.f, 0.f, 0.f, 0.f};
+                const float2 sc2 = make_float2(scale_log2, scale_log2), mn2 = make_float2(mneg, mneg);
+                float2 ps[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
 #pragma unroll
                 for (int i = 0; i < 4; ++i)
 #pragma unroll
                     for (int e = 0; e < 32; e += 2) {
-                        const float p0 = ptx::ex2(fmaf(__uint_as_float(sv[i][e]), scale_log2, mneg));
-                        const float p1 = ptx::ex2(fmaf(__uint_as_float(sv[i][e + 1]), scale_log2, mneg));
-                        ps[(e >> 1) & 3] += p0 + p1;
-                        sv[i >> 1][(i & 1) * 16 + (e >> 1)] = ptx::pack_bf16x2(p0, p1);   // packed P: 64 registers
+                        // packed fp32x2 FMA / ADD (sm_100): one instruction per pair of scores
+                        const float2 x = __ffma2_rn(make_float2(__uint_as_float(sv[i][e]), __uint_as_float(sv[i][e + 1])), sc2, mn2);
+                        const float2 p = make_float2(ptx::ex2(x.x), ptx::ex2(x.y));
+                        ps[(e >> 1) & 3] = __fadd2_rn(ps[(e >> 1) & 3], p);
+                        sv[i >> 1][(i & 1) * 16 + (e >> 1)] = ptx::pack_bf16x2(p.x, p.y);   // packed P: 64 registers
                     }
-                l_sum = l_sum * alpha + ((ps[0] + ps[1]) + (ps[2] + ps[3]));
+                l_sum = l_sum * alpha + (((ps[0].x + ps[0].y) + (ps[1].x + ps[1].y)) + ((ps[2].x + ps[2].y) + (ps[3].x + ps[3].y)));
 
                 if (j > 0 && __any_sync(0xffffffffu, grow)) {
                     // O_w holds the sum up to tile j-1: S_FULL(j) was committed after PV(j-1), so it is complete
@@ -318,37 +390,17 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 ptx::tc_fence_before();
                 ptx::mbar_arrive(bar(BAR_P_FULL + wg));
             }
-
-            // ---- epilogue: O / l -> bf16 -> global ----
-            ptx::mbar_wait(bar(BAR_PV_DONE + wg), (cnt - 1u) & 1u);
-            ptx::tc_fence_after();
-            const float inv_l = 1.f / l_sum;
-            __nv_bfloat16* orow = out + ((size_t)(w.tok0 + tl) * Hq + (size_t)w.kvh * g + hh) * D;
-#pragma unroll
-            for (int i = 0; i < D / 32; ++i) {
-                uint32_t o[32];
-                ptx::tmem_ld32(tO + i * 32, o);
-                ptx::tmem_ld_wait();
-                if (row_valid) {
-#pragma unroll
-                    for (int e = 0; e < 32; e += 8) {
-                        uint4 pk;
-                        pk.x = ptx::pack_bf16x2(__uint_as_float(o[e]) * inv_l, __uint_as_float(o[e + 1]) * inv_l);
-                        pk.y = ptx::pack_bf16x2(__uint_as_float(o[e + 2]) * inv_l, __uint_as_float(o[e + 3]) * inv_l);
-                        pk.z = ptx::pack_bf16x2(__uint_as_float(o[e + 4]) * inv_l, __uint_as_float(o[e + 5]) * inv_l);
-                        pk.w = ptx::pack_bf16x2(__uint_as_float(o[e + 6]) * inv_l, __uint_as_float(o[e + 7]) * inv_l);
-                        *reinterpret_cast<uint4*>(orow + i * 32 + e) = pk;
-                    }
-                }
-            }
-            ptx::tc_fence_before();
-            ptx::mbar_arrive(bar(BAR_O_EMPTY + wg));
+            // hand the row sum to the epilogue group and go on to the next item
+            ptx::mbar_wait(bar(BAR_L_EMPTY + wg), (litem & 1u) ^ 1u);
+            ptx::st_shared_f32(sbase + L::kL + (wg * 128 + row) * 4, l_sum);
+            ptx::mbar_arrive(bar(BAR_L_FULL + wg));
+            ++litem;
         }
     }
 
     ptx::tc_fence_before();
     __syncthreads();
-    if (warp == 8) {
+    if (warp == 12) {
         ptx::tc_fence_after();
         ptx::tmem_dealloc(tmem, 512);
     }
