@@ -161,29 +161,39 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                     blk = blk_next;
                 }
             }
-        } else if (warp == 12 && lane == 0) {
-            // ================================ MMA issuer (one thread) ================================
+        } else if (warp == 12) {
+            // ================================ MMA issuer ================================
+            // The whole warp runs the control flow (so addresses and descriptors stay in uniform registers); one elected
+            // lane issues the MMAs and commits.
             constexpr uint32_t kIdescQK = ptx::umma_idesc_bf16(kTileM, kTileN, 0, 0);
             constexpr uint32_t kIdescPV = ptx::umma_idesc_bf16(kTileM, D, 0, 1);
             constexpr uint32_t kGroupStride = (D / 64) * 1024;        // bytes between 8-key groups of a K/V tile
             uint32_t it = 0, cnt0 = 0, cnt1 = 0, oitem0 = 0, oitem1 = 0;
             int item_n = 0;
+            const uint64_t qdesc0 = ptx::umma_desc_sw128(sbase + L::kQ, 16, 1024);
+            const uint64_t kdesc0 = ptx::umma_desc_sw128(sbase + L::kRing, 16, kGroupStride);
+            const uint64_t vdesc0 = ptx::umma_desc_sw128(sbase + L::kRing, 1024, kGroupStride);
             auto issue_qk = [&](int w, uint32_t slot) {
-                const uint32_t qb = sbase + L::kQ + w * L::kQBytes, kb = sbase + L::kRing + slot * L::kKVBytes;
+                const uint64_t qd = qdesc0 + (uint64_t)((w * L::kQBytes) >> 4), kd = kdesc0 + (uint64_t)((slot * L::kKVBytes) >> 4);
+                const uint32_t ts = tmem + (uint32_t)w * 128u;
 #pragma unroll
-                for (int ks = 0; ks < D / 16; ++ks) {
-                    const uint64_t a = ptx::umma_desc_sw128(qb + (ks >> 2) * (kTileM * 128) + (ks & 3) * 32, 16, 1024);
-                    const uint64_t b = ptx::umma_desc_sw128(kb + (ks >> 2) * 1024 + (ks & 3) * 32, 16, kGroupStride);
-                    ptx::umma_ss(tmem + (uint32_t)w * 128u, a, b, kIdescQK, ks > 0);
-                }
+                for (int ks = 0; ks < D / 16; ++ks)
+                    ptx::umma_ss(ts, qd + (uint64_t)(((ks >> 2) * (kTileM * 128) + (ks & 3) * 32) >> 4),
+                                 kd + (uint64_t)(((ks >> 2) * 1024 + (ks & 3) * 32) >> 4), kIdescQK, ks > 0);
                 ptx::umma_commit(bar(BAR_S_FULL + w));
             };
             auto issue_pv = [&](int w, uint32_t slot, int ksteps, bool first) {
-                const uint32_t vb = sbase + L::kRing + slot * L::kKVBytes;
-                for (int ks = 0; ks < ksteps; ++ks) {
-                    const uint64_t b = ptx::umma_desc_sw128(vb + ks * 2 * kGroupStride, 1024, kGroupStride);
-                    ptx::umma_ts(tmem + 256u + (uint32_t)w * 128u, tmem + (uint32_t)w * 128u + (uint32_t)ks * 8u, b, kIdescPV,
-                                 (!first || ks > 0) ? 1u : 0u);
+                const uint64_t vd = vdesc0 + (uint64_t)((slot * L::kKVBytes) >> 4);
+                const uint32_t to = tmem + 256u + (uint32_t)w * 128u, tp = tmem + (uint32_t)w * 128u;
+                if (ksteps == 8) {
+#pragma unroll
+                    for (int ks = 0; ks < 8; ++ks)
+                        ptx::umma_ts(to, tp + (uint32_t)ks * 8u, vd + (uint64_t)((ks * 2 * kGroupStride) >> 4), kIdescPV,
+                                     (!first || ks > 0) ? 1u : 0u);
+                } else {
+                    for (int ks = 0; ks < ksteps; ++ks)
+                        ptx::umma_ts(to, tp + (uint32_t)ks * 8u, vd + (uint64_t)((ks * 2 * kGroupStride) >> 4), kIdescPV,
+                                     (!first || ks > 0) ? 1u : 0u);
                 }
                 ptx::umma_commit(bar(BAR_PV_DONE + w));
             };
@@ -201,50 +211,51 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 ptx::mbar_wait(bar(BAR_Q_FULL), (uint32_t)item_n & 1u);
                 wait_full(it);
                 ptx::tc_fence_after();
-                issue_qk(0, slot_of(it));
-                if (n1) issue_qk(1, slot_of(it));
-                release(it);
-                if (nt == 1) ptx::umma_commit(bar(BAR_Q_EMPTY));
+                if (ptx::elect_one()) {
+                    issue_qk(0, slot_of(it));
+                    if (n1) issue_qk(1, slot_of(it));
+                    release(it);
+                    if (nt == 1) ptx::umma_commit(bar(BAR_Q_EMPTY));
+                }
+                __syncwarp();
                 for (int j = 0; j < nt; ++j) {
                     const uint32_t iv = it + 2 * j + 1, ikn = it + 2 * j + 2;
                     const int left = nkv - j * kTileN;
                     const int ksteps = left >= kTileN ? 8 : (left + 15) >> 4;   // skip 16-key steps with no valid key
                     wait_full(iv);
-                    bool k_ready = false;
-                    // ---- Q tile 0 ----
+                    if (j + 1 < nt) wait_full(ikn);
+                    // ---- Q tile 0: O0 += P0 V(j), then S0 = Q0 K(j+1)^T ----
                     if (j < n0) {
                         ptx::mbar_wait(bar(BAR_P_FULL + 0), cnt0 & 1u);
                         if (j == 0) ptx::mbar_wait(bar(BAR_O_EMPTY + 0), (oitem0 & 1u) ^ 1u);
                         ptx::tc_fence_after();
-                        issue_pv(0, slot_of(iv), ksteps, j == 0);
+                        if (ptx::elect_one()) {
+                            issue_pv(0, slot_of(iv), ksteps, j == 0);
+                            if (j + 1 < n0) issue_qk(0, slot_of(ikn));
+                        }
+                        __syncwarp();
                         ++cnt0;
-                    }
-                    if (j + 1 < n0) {
-                        wait_full(ikn);
-                        ptx::tc_fence_after();
-                        k_ready = true;
-                        issue_qk(0, slot_of(ikn));
                     }
                     // ---- Q tile 1 ----
                     if (j < n1) {
                         ptx::mbar_wait(bar(BAR_P_FULL + 1), cnt1 & 1u);
                         if (j == 0) ptx::mbar_wait(bar(BAR_O_EMPTY + 1), (oitem1 & 1u) ^ 1u);
                         ptx::tc_fence_after();
-                        issue_pv(1, slot_of(iv), ksteps, j == 0);
+                        if (ptx::elect_one()) {
+                            issue_pv(1, slot_of(iv), ksteps, j == 0);
+                            if (j + 1 < n1) issue_qk(1, slot_of(ikn));
+                        }
+                        __syncwarp();
                         ++cnt1;
                     }
-                    if (j + 1 < n1) {
-                        if (!k_ready) {
-                            wait_full(ikn);
-                            ptx::tc_fence_after();
+                    if (ptx::elect_one()) {
+                        release(iv);
+                        if (j + 1 < nt) {
+                            release(ikn);
+                            if (j + 2 == nt) ptx::umma_commit(bar(BAR_Q_EMPTY));
                         }
-                        issue_qk(1, slot_of(ikn));
                     }
-                    release(iv);
-                    if (j + 1 < nt) {
-                        release(ikn);
-                        if (j + 2 == nt) ptx::umma_commit(bar(BAR_Q_EMPTY));
-                    }
+                    __syncwarp();
                 }
                 it += 2u * (uint32_t)nt;
                 oitem0 += 1;
