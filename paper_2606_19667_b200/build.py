@@ -37,6 +37,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     cmd = [_nvcc(), "-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
            "-shared", "-Xcompiler", "-fPIC,-Wall,-Wno-unused-function", "-I", os.path.join(ROOT, "include"), "-I", CSRC,
            "-x", "cu"] + [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB]
+    cmd[1:1] = os.environ.get("CW_NVCC_FLAGS", "").split()      # experiments only (e.g. -DCW_EXP_NOLOAD)
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     r = subprocess.run(cmd, capture_output=True, text=True)

@@ -7,7 +7,7 @@
 // heads and both Q tiles (M = 256 per CTA), and a short query-only suffix still fills the MMA.
 //
 // Persistent CTAs (one per SM, 512 threads = 4 warpgroups), static round-robin over a host-built item list,
-// warp-specialised, mbarrier pipelines only; registers are re-balanced with setmaxnreg (softmax 192, epilogue 80, rest 48):
+// warp-specialised, mbarrier pipelines only; registers are re-balanced with setmaxnreg (softmax 192, epilogue 64, MMA+loader 64):
 //   warps 0-3   softmax + lazy rescale of Q tile 0 (thread i owns TMEM lane i = packed row i)
 //   warps 4-7   the same for Q tile 1 — the two groups ping-pong: while one does exp on S_w, the tensor core runs the
 //               other tile's PV and next QK^T
@@ -50,16 +50,49 @@ struct Smem {
 };
 
 // barrier slots (ring FULL[s] at BAR_RING + s, EMPTY[s] at BAR_RING + kStages + s)
-enum { BAR_Q_FULL = 0, BAR_Q_EMPTY = 1, BAR_S_FULL = 2, BAR_P_FULL = 4, BAR_PV_DONE = 6, BAR_O_EMPTY = 8, BAR_L_FULL = 10,
-       BAR_L_EMPTY = 12, BAR_RING = 14 };
+enum { BAR_Q_FULL = 0, BAR_Q_EMPTY = 2, BAR_S_FULL = 4, BAR_P_FULL = 6, BAR_PV_DONE = 8, BAR_O_EMPTY = 10, BAR_L_FULL = 12,
+       BAR_L_EMPTY = 14, BAR_RING = 16 };
 
+// Work item, 8 ints: {pos0, ntok0, ntok1, tok0 | r, kvh, q_off16, 0}.  The first int4 is all the softmax and MMA warps need.
+//   pos0: absolute position of the first token; ntok0/1: tokens of Q tile 0/1; tok0: index of the first token in [0,T);
+//   q_off16: offset of Q tile 0 inside q_roped in 16-byte units.
 struct Item {
-    int r, kvh, tok0, pos0, ntok0, ntok1, q_off16;   // q_off16: offset of Q tile 0 inside q_roped in 16-byte units
+    int pos0, ntok0, ntok1, tok0, r, kvh, q_off16;
 };
-
+// volatile: the prefetch of the next item must stay where it is written (ptxas otherwise sinks it next to its first use)
+__device__ __forceinline__ int4 ld_item_half(const int4* p) {
+    int4 v;
+    asm volatile("ld.global.nc.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ Item load_item(const int4* __restrict__ work, int idx) {
-    const int4 a = __ldg(work + 2 * idx), b = __ldg(work + 2 * idx + 1);
+    const int4 a = ld_item_half(work + 2 * idx), b = ld_item_half(work + 2 * idx + 1);
     return Item{a.x, a.y, a.z, a.w, b.x, b.y, b.z};
+}
+__device__ __forceinline__ Item load_item_head(const int4* __restrict__ work, int idx) {   // pos0, ntok0, ntok1, tok0 only
+    const int4 a = ld_item_half(work + 2 * idx);
+    return Item{a.x, a.y, a.z, a.w, 0, 0, 0};
+}
+
+// exp2 on the FMA pipe for a share of the scores (the MUFU unit, 16 exp2 / clk / SM, is the softmax bottleneck):
+// 2^x = 2^round(x) * 2^f, f = x - round(x) in [-0.5, 0.5]; 2^f by a degree-3 polynomial (max rel. error 7.8e-5, P is
+// rounded to bf16 = 3.9e-3 afterwards); round(x) through the 1.5*2^23 magic constant, spliced into the exponent field.
+constexpr int kPolyPeriod = 4;       // of every kPolyPeriod score pairs ...
+constexpr int kPolyCount = 2;        // ... this many use the polynomial
+__device__ __forceinline__ float2 exp2_poly2(float2 x) {
+    const float kMagic = 12582912.f;
+    x.x = fmaxf(x.x, -125.f);
+    x.y = fmaxf(x.y, -125.f);
+    const float2 t = __fadd2_rn(x, make_float2(kMagic, kMagic));
+    const float2 r = __fadd2_rn(t, make_float2(-kMagic, -kMagic));
+    const float2 f = __fadd2_rn(x, make_float2(-r.x, -r.y));
+    float2 p = __ffma2_rn(make_float2(0.05508868396282196f, 0.05508868396282196f), f,
+                          make_float2(0.24260404706001282f, 0.24260404706001282f));
+    p = __ffma2_rn(p, f, make_float2(0.6932762265205383f, 0.6932762265205383f));
+    p = __ffma2_rn(p, f, make_float2(0.9999289512634277f, 0.9999289512634277f));
+    p.x = __int_as_float(__float_as_int(p.x) + (__float_as_int(t.x) << 23));
+    p.y = __int_as_float(__float_as_int(p.y) + (__float_as_int(t.y) << 23));
+    return p;
 }
 
 __device__ __forceinline__ int tiles_for(int nkv) { return (nkv + kTileN - 1) / kTileN; }
@@ -86,9 +119,9 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
     const int R = tpt * g;               // rows of a full Q tile
 
     if (threadIdx.x == 0) {
-        ptx::mbar_init(bar(BAR_Q_FULL), 1);
-        ptx::mbar_init(bar(BAR_Q_EMPTY), 1);
         for (int w = 0; w < 2; ++w) {
+            ptx::mbar_init(bar(BAR_Q_FULL + w), 1);
+            ptx::mbar_init(bar(BAR_Q_EMPTY + w), 1);
             ptx::mbar_init(bar(BAR_S_FULL + w), 1);
             ptx::mbar_init(bar(BAR_P_FULL + w), 128);
             ptx::mbar_init(bar(BAR_PV_DONE + w), 1);
@@ -106,16 +139,18 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
     const uint32_t tmem = *tmem_slot;
 
     if (warp >= 12) {
-        ptx::setmaxnreg_dec<48>();
+        ptx::setmaxnreg_dec<64>();
         if (warp == 13) {
             // ================================ loader ================================
+            // Ring order per item: K(0) V(0) K(1) V(1) ...; the item's two Q tiles are loaded after K(0), V(0) so that
+            // the MMA warp can chain QK(0) of this item right behind the last PV of the previous one.
             constexpr uint32_t kBlockBytes = 16 * D * 2;
-            uint32_t it = 0;
-            int item_n = 0;
+            uint32_t it = 0, qcnt0 = 0, qcnt1 = 0;
             Item nxt = load_item(work, blockIdx.x);
-            for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x, ++item_n) {
+            for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
                 const Item w = nxt;
-                if (idx + (int)gridDim.x < num_items) nxt = load_item(work, idx + gridDim.x);
+                const bool has_next = idx + (int)gridDim.x < num_items;
+                if (has_next) nxt = load_item(work, idx + gridDim.x);
                 const int rows0 = w.ntok0 * g, rows1 = w.ntok1 * g;
                 const int nkv = w.pos0 + w.ntok0 + w.ntok1;
                 const int nt = tiles_for(nkv);
@@ -125,25 +160,7 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                     const int nb = left >= kTileN ? 8 : (left + 15) >> 4;
                     return lane < nb ? __ldg(table + j * 8 + lane) : 0;
                 };
-                int blk = load_ids(0);
-                ptx::mbar_wait(bar(BAR_Q_EMPTY), ((uint32_t)item_n & 1u) ^ 1u);
-                if (lane == 0) {
-                    ptx::mbar_arrive_expect_tx(bar(BAR_Q_FULL), (uint32_t)((rows0 + rows1) * D * 2));
-                    const char* src = reinterpret_cast<const char*>(q_roped) + (size_t)w.q_off16 * 16;
-#pragma unroll
-                    for (int h = 0; h < D / 64; ++h)
-                        ptx::bulk_g2s(sbase + L::kQ + h * (kTileM * 128), src + (size_t)h * rows0 * 128,
-                                      (uint32_t)rows0 * 128u, bar(BAR_Q_FULL));
-                    if (rows1) {
-                        const char* src1 = src + (size_t)R * D * 2;      // tile 0 is full whenever tile 1 exists
-#pragma unroll
-                        for (int h = 0; h < D / 64; ++h)
-                            ptx::bulk_g2s(sbase + L::kQ + L::kQBytes + h * (kTileM * 128), src1 + (size_t)h * rows1 * 128,
-                                          (uint32_t)rows1 * 128u, bar(BAR_Q_FULL));
-                    }
-                }
-                for (int j = 0; j < nt; ++j) {
-                    const int blk_next = j + 1 < nt ? load_ids(j + 1) : 0;
+                auto load_kv = [&](int j, int blk) {
                     const int left = nkv - j * kTileN;
                     const int nblk = left >= kTileN ? 8 : (left + 15) >> 4;
                     const size_t src_off = ((size_t)blk * Hkv + w.kvh) * (16 * D);
@@ -151,6 +168,13 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                     for (int kv = 0; kv < 2; ++kv) {
                         const uint32_t s = it % NS, ph = (it / NS) & 1u;
                         ptx::mbar_wait(bar(BAR_RING + NS + s), ph ^ 1u);
+#ifdef CW_EXP_NOLOAD   // timing experiment only (wrong results): K/V tiles are loaded for the first ring fill, then faked
+                        if (it >= NS) {
+                            if (lane == 0) ptx::mbar_arrive(bar(BAR_RING + s));
+                            ++it;
+                            continue;
+                        }
+#endif
                         if (lane == 0) ptx::mbar_arrive_expect_tx(bar(BAR_RING + s), kBlockBytes * (uint32_t)nblk);
                         __syncwarp();
                         if (lane < nblk)
@@ -158,33 +182,76 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                                           (kv == 0 ? k_pool : v_pool) + src_off, kBlockBytes, bar(BAR_RING + s));
                         ++it;
                     }
+                };
+                int blk = load_ids(0);
+                int blk_next = nt > 1 ? load_ids(1) : 0;
+                load_kv(0, blk);
+                // Q tiles: each buffer is free once the previous item's last QK^T of that tile has completed
+                const char* src = reinterpret_cast<const char*>(q_roped) + (size_t)w.q_off16 * 16;
+                ptx::mbar_wait(bar(BAR_Q_EMPTY + 0), (qcnt0 & 1u) ^ 1u);
+                ++qcnt0;
+                if (lane == 0) {
+                    ptx::mbar_arrive_expect_tx(bar(BAR_Q_FULL + 0), (uint32_t)(rows0 * D * 2));
+#pragma unroll
+                    for (int h = 0; h < D / 64; ++h)
+                        ptx::bulk_g2s(sbase + L::kQ + h * (kTileM * 128), src + (size_t)h * rows0 * 128,
+                                      (uint32_t)rows0 * 128u, bar(BAR_Q_FULL + 0));
+                }
+                if (rows1) {
+                    ptx::mbar_wait(bar(BAR_Q_EMPTY + 1), (qcnt1 & 1u) ^ 1u);
+                    ++qcnt1;
+                    if (lane == 0) {
+                        const char* src1 = src + (size_t)R * D * 2;      // tile 0 is full whenever tile 1 exists
+                        ptx::mbar_arrive_expect_tx(bar(BAR_Q_FULL + 1), (uint32_t)(rows1 * D * 2));
+#pragma unroll
+                        for (int h = 0; h < D / 64; ++h)
+                            ptx::bulk_g2s(sbase + L::kQ + L::kQBytes + h * (kTileM * 128), src1 + (size_t)h * rows1 * 128,
+                                          (uint32_t)rows1 * 128u, bar(BAR_Q_FULL + 1));
+                    }
+                }
+                if (has_next && lane == 0)   // pull the next item's Q tiles into L2 while this item computes
+                    ptx::bulk_prefetch_l2(reinterpret_cast<const char*>(q_roped) + (size_t)nxt.q_off16 * 16,
+                                          (uint32_t)((nxt.ntok0 + nxt.ntok1) * g * D * 2));
+                for (int j = 1; j < nt; ++j) {
                     blk = blk_next;
+                    blk_next = j + 1 < nt ? load_ids(j + 1) : 0;
+                    load_kv(j, blk);
                 }
             }
         } else if (warp == 12) {
             // ================================ MMA issuer ================================
             // The whole warp runs the control flow (so addresses and descriptors stay in uniform registers); one elected
-            // lane issues the MMAs and commits.
+            // lane issues the MMAs and commits.  The items of this CTA form one continuous stream: QK^T(0) of the next
+            // item is issued right behind the last PV of the current one, so the ping-pong never drains between items.
             constexpr uint32_t kIdescQK = ptx::umma_idesc_bf16(kTileM, kTileN, 0, 0);
             constexpr uint32_t kIdescPV = ptx::umma_idesc_bf16(kTileM, D, 0, 1);
             constexpr uint32_t kGroupStride = (D / 64) * 1024;        // bytes between 8-key groups of a K/V tile
-            uint32_t it = 0, cnt0 = 0, cnt1 = 0, oitem0 = 0, oitem1 = 0;
-            int item_n = 0;
+            uint32_t it = 0, cnt0 = 0, cnt1 = 0, oitem0 = 0, oitem1 = 0, qf0 = 0, qf1 = 0;
             const uint64_t qdesc0 = ptx::umma_desc_sw128(sbase + L::kQ, 16, 1024);
             const uint64_t kdesc0 = ptx::umma_desc_sw128(sbase + L::kRing, 16, kGroupStride);
             const uint64_t vdesc0 = ptx::umma_desc_sw128(sbase + L::kRing, 1024, kGroupStride);
-            auto issue_qk = [&](int w, uint32_t slot) {
+            auto slot_of = [&](uint32_t i) { return i % NS; };
+            auto wait_full = [&](uint32_t i) { ptx::mbar_wait(bar(BAR_RING + slot_of(i)), (i / NS) & 1u); };
+            auto release = [&](uint32_t i) { ptx::umma_commit(bar(BAR_RING + NS + slot_of(i))); };
+            // S_w = Q_w K^T; `last`: no further QK^T of this item reads Q_w, so its buffer is handed back to the loader
+            auto issue_qk = [&](int w, uint32_t slot, bool last) {
                 const uint64_t qd = qdesc0 + (uint64_t)((w * L::kQBytes) >> 4), kd = kdesc0 + (uint64_t)((slot * L::kKVBytes) >> 4);
                 const uint32_t ts = tmem + (uint32_t)w * 128u;
+#ifndef CW_EXP_NOQK
 #pragma unroll
                 for (int ks = 0; ks < D / 16; ++ks)
                     ptx::umma_ss(ts, qd + (uint64_t)(((ks >> 2) * (kTileM * 128) + (ks & 3) * 32) >> 4),
                                  kd + (uint64_t)(((ks >> 2) * 1024 + (ks & 3) * 32) >> 4), kIdescQK, ks > 0);
+#endif
                 ptx::umma_commit(bar(BAR_S_FULL + w));
+                if (last) ptx::umma_commit(bar(BAR_Q_EMPTY + w));
             };
             auto issue_pv = [&](int w, uint32_t slot, int ksteps, bool first) {
                 const uint64_t vd = vdesc0 + (uint64_t)((slot * L::kKVBytes) >> 4);
                 const uint32_t to = tmem + 256u + (uint32_t)w * 128u, tp = tmem + (uint32_t)w * 128u;
+#ifdef CW_EXP_NOPV
+                ksteps = 0;
+#endif
                 if (ksteps == 8) {
 #pragma unroll
                     for (int ks = 0; ks < 8; ++ks)
@@ -197,33 +264,42 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 }
                 ptx::umma_commit(bar(BAR_PV_DONE + w));
             };
-            Item nxt = load_item(work, blockIdx.x);
-            for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x, ++item_n) {
+            // first QK^T of an item's tiles (K(0) sits at ring index i0); called once up front and then from inside the
+            // last iteration of the previous item
+            auto open_tile = [&](int w, const Item& x, uint32_t i0) {
+                const int ntok = w ? x.ntok1 : x.ntok0;
+                if (ntok == 0) return;
+                uint32_t& qf = w ? qf1 : qf0;
+                ptx::mbar_wait(bar(BAR_Q_FULL + w), qf & 1u);
+                ++qf;
+                ptx::tc_fence_after();
+                const int n_w = tiles_for(x.pos0 + w * tpt + ntok);
+                if (ptx::elect_one()) issue_qk(w, slot_of(i0), n_w == 1);
+                __syncwarp();
+            };
+            Item nxt = load_item_head(work, blockIdx.x);
+            if ((int)blockIdx.x < num_items) {
+                wait_full(0);
+                open_tile(0, nxt, 0);
+                open_tile(1, nxt, 0);
+                if (ptx::elect_one()) release(0);
+                __syncwarp();
+            }
+            for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
                 const Item w = nxt;
-                if (idx + (int)gridDim.x < num_items) nxt = load_item(work, idx + gridDim.x);
+                const bool has_next = idx + (int)gridDim.x < num_items;
+                if (has_next) nxt = load_item_head(work, idx + gridDim.x);
                 const int nkv0 = w.pos0 + w.ntok0, nkv1 = nkv0 + w.ntok1;
                 const int n0 = tiles_for(nkv0), n1 = w.ntok1 ? tiles_for(nkv1) : 0;
                 const int nt = n1 ? n1 : n0;
                 const int nkv = w.ntok1 ? nkv1 : nkv0;
-                auto slot_of = [&](uint32_t i) { return i % NS; };
-                auto wait_full = [&](uint32_t i) { ptx::mbar_wait(bar(BAR_RING + slot_of(i)), (i / NS) & 1u); };
-                auto release = [&](uint32_t i) { ptx::umma_commit(bar(BAR_RING + NS + slot_of(i))); };
-                ptx::mbar_wait(bar(BAR_Q_FULL), (uint32_t)item_n & 1u);
-                wait_full(it);
-                ptx::tc_fence_after();
-                if (ptx::elect_one()) {
-                    issue_qk(0, slot_of(it));
-                    if (n1) issue_qk(1, slot_of(it));
-                    release(it);
-                    if (nt == 1) ptx::umma_commit(bar(BAR_Q_EMPTY));
-                }
-                __syncwarp();
                 for (int j = 0; j < nt; ++j) {
-                    const uint32_t iv = it + 2 * j + 1, ikn = it + 2 * j + 2;
+                    const uint32_t iv = it + 2 * j + 1, ikn = it + 2 * j + 2;   // ikn: K(j+1), or K(0) of the next item
+                    const bool last_iter = j + 1 == nt;
                     const int left = nkv - j * kTileN;
                     const int ksteps = left >= kTileN ? 8 : (left + 15) >> 4;   // skip 16-key steps with no valid key
                     wait_full(iv);
-                    if (j + 1 < nt) wait_full(ikn);
+                    if (!last_iter || has_next) wait_full(ikn);
                     // ---- Q tile 0: O0 += P0 V(j), then S0 = Q0 K(j+1)^T ----
                     if (j < n0) {
                         ptx::mbar_wait(bar(BAR_P_FULL + 0), cnt0 & 1u);
@@ -231,11 +307,12 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                         ptx::tc_fence_after();
                         if (ptx::elect_one()) {
                             issue_pv(0, slot_of(iv), ksteps, j == 0);
-                            if (j + 1 < n0) issue_qk(0, slot_of(ikn));
+                            if (j + 1 < n0) issue_qk(0, slot_of(ikn), j + 2 == n0);
                         }
                         __syncwarp();
                         ++cnt0;
                     }
+                    if (last_iter && has_next) open_tile(0, nxt, ikn);
                     // ---- Q tile 1 ----
                     if (j < n1) {
                         ptx::mbar_wait(bar(BAR_P_FULL + 1), cnt1 & 1u);
@@ -243,17 +320,15 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                         ptx::tc_fence_after();
                         if (ptx::elect_one()) {
                             issue_pv(1, slot_of(iv), ksteps, j == 0);
-                            if (j + 1 < n1) issue_qk(1, slot_of(ikn));
+                            if (j + 1 < n1) issue_qk(1, slot_of(ikn), j + 2 == n1);
                         }
                         __syncwarp();
                         ++cnt1;
                     }
+                    if (last_iter && has_next) open_tile(1, nxt, ikn);
                     if (ptx::elect_one()) {
                         release(iv);
-                        if (j + 1 < nt) {
-                            release(ikn);
-                            if (j + 2 == nt) ptx::umma_commit(bar(BAR_Q_EMPTY));
-                        }
+                        if (!last_iter || has_next) release(ikn);
                     }
                     __syncwarp();
                 }
@@ -265,7 +340,7 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
         __syncwarp();
     } else if (warp >= 8) {
         // ================================ epilogue (warps 8-11): O_w / l_w -> bf16 -> global ================================
-        ptx::setmaxnreg_dec<80>();
+        ptx::setmaxnreg_dec<64>();
         const int row = threadIdx.x & 127;                 // TMEM lane == packed row within a tile
         const uint32_t lane_base = ((uint32_t)((warp & 3) * 32)) << 16;
         const int tdiv = row / g, hh = row - tdiv * g;
@@ -319,10 +394,10 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
         const uint32_t tO = tmem + 256u + (uint32_t)wg * 128u + lane_base;
         const int tl = wg * tpt + row / g;                 // token of this row inside the item
         uint32_t cnt = 0, litem = 0;
-        Item nxt = load_item(work, blockIdx.x);
+        Item nxt = load_item_head(work, blockIdx.x);
         for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
             const Item w = nxt;
-            if (idx + (int)gridDim.x < num_items) nxt = load_item(work, idx + gridDim.x);
+            if (idx + (int)gridDim.x < num_items) nxt = load_item_head(work, idx + gridDim.x);
             const int ntok = wg ? w.ntok1 : w.ntok0;
             if (ntok == 0) continue;
             const int limit = w.pos0 + tl;                 // last visible key (inclusive); rows past the tile end are never stored
@@ -332,6 +407,12 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
             for (int j = 0; j < n_tiles; ++j, ++cnt) {
                 ptx::mbar_wait(bar(BAR_S_FULL + wg), cnt & 1u);
                 ptx::tc_fence_after();
+#ifdef CW_EXP_NOSOFTMAX   // timing experiment only (wrong results): the softmax group only hands the tile back
+                l_sum = 1.f;
+                ptx::tc_fence_before();
+                ptx::mbar_arrive(bar(BAR_P_FULL + wg));
+                continue;
+#endif
                 uint32_t sv[4][32];
 #pragma unroll
                 for (int i = 0; i < 4; ++i) ptx::tmem_ld32(tS + i * 32, sv[i]);
@@ -374,7 +455,9 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                     for (int e = 0; e < 32; e += 2) {
                         // packed fp32x2 FMA / ADD (sm_100): one instruction per pair of scores
                         const float2 x = __ffma2_rn(make_float2(__uint_as_float(sv[i][e]), __uint_as_float(sv[i][e + 1])), sc2, mn2);
-                        const float2 p = make_float2(ptx::ex2(x.x), ptx::ex2(x.y));
+                        float2 p;
+                        if (((e >> 1) % kPolyPeriod) < kPolyCount) p = exp2_poly2(x);        // FMA pipe
+                        else p = make_float2(ptx::ex2(x.x), ptx::ex2(x.y));                  // MUFU (16 / clk / SM)
                         ps[(e >> 1) & 3] = __fadd2_rn(ps[(e >> 1) & 3], p);
                         sv[i >> 1][(i & 1) * 16 + (e >> 1)] = ptx::pack_bf16x2(p.x, p.y);   // packed P: 64 registers
                     }
@@ -457,7 +540,7 @@ int64_t attn_build_schedule(const cw_config& cfg, const int32_t* h_cu, const int
                 const int tok0 = t * 2 * tpt;
                 const int ntok0 = std::min(tpt, s - tok0), ntok1 = std::max(0, std::min(tpt, s - tok0 - tpt));
                 const int64_t q_off = ((int64_t)h_cu[r] * Hq + (int64_t)kvh * s * g) * D + (int64_t)t * 2 * R * D;   // elements
-                const int32_t item[kWorkInts] = {r, kvh, h_cu[r] + tok0, h_nc[r] + tok0, ntok0, ntok1, (int32_t)(q_off / 8), 0};
+                const int32_t item[kWorkInts] = {h_nc[r] + tok0, ntok0, ntok1, h_cu[r] + tok0, r, kvh, (int32_t)(q_off / 8), 0};
                 work.insert(work.end(), item, item + kWorkInts);
             }
     }
