@@ -328,7 +328,7 @@ WsLayout ws_layout(const cw_config& c, int32_t B, int32_t T, int32_t max_blocks)
     const int g = c.num_q_heads / c.num_kv_heads;
     const int tpt2 = 2 * (128 / g);
     const int64_t max_items = (((int64_t)T + tpt2 - 1) / tpt2 + B) * c.num_kv_heads;
-    w.work = o; o += align256(max_items * 32);
+    w.work = o; o += align256((max_items + 1) * 32);
     w.total = o;
     return w;
 }

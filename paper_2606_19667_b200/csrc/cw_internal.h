@@ -112,5 +112,5 @@ int64_t attn_work_ints(const cw_config& cfg, const int32_t* h_cu, int32_t B);
 int64_t attn_build_schedule(const cw_config& cfg, const int32_t* h_cu, const int32_t* h_nc, int32_t B,
                             std::vector<int32_t>& work);
 int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* tables, int32_t max_blocks,
-                        const int32_t* d_work, int64_t num_items, int num_sms, void* stream);
+                        int32_t* d_work, int64_t num_items, int num_sms, void* stream);
 }  // namespace cw

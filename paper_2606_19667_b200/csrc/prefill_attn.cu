@@ -6,7 +6,7 @@
 // heads that share the kv head, packed into the M dimension (row = token*g + head), so one K/V tile read feeds all g
 // heads and both Q tiles (M = 256 per CTA), and a short query-only suffix still fills the MMA.
 //
-// Persistent CTAs (one per SM, 512 threads = 4 warpgroups), static round-robin over a host-built item list,
+// Persistent CTAs (one per SM, 512 threads = 4 warpgroups) claiming items from a host-built list with an atomic counter,
 // warp-specialised, mbarrier pipelines only; registers are re-balanced with setmaxnreg (softmax 192, epilogue 64, MMA+loader 64):
 //   warps 0-3   softmax + lazy rescale of Q tile 0 (thread i owns TMEM lane i = packed row i)
 //   warps 4-7   the same for Q tile 1 — the two groups ping-pong: while one does exp on S_w, the tensor core runs the
@@ -45,13 +45,16 @@ struct Smem {
     static constexpr int kQ = 0;
     static constexpr int kRing = kQ + 2 * kQBytes;
     static constexpr int kBar = kRing + kStages * kKVBytes;   // mbarriers (8 B each), then the TMEM slot
-    static constexpr int kL = kBar + 256;                     // l_sum hand-off softmax -> epilogue: float [2][128]
-    static constexpr int kTotal = kL + 1024;
+    static constexpr int kL = kBar + 512;                     // l_sum hand-off softmax -> epilogue: float [2][128]
+    static constexpr int kSched = kL + 1024;                  // item ring: kSchedSlots x 8 ints, filled by the loader warp
+    static constexpr int kTotal = kSched + 128;
 };
 
 // barrier slots (ring FULL[s] at BAR_RING + s, EMPTY[s] at BAR_RING + kStages + s)
 enum { BAR_Q_FULL = 0, BAR_Q_EMPTY = 2, BAR_S_FULL = 4, BAR_P_FULL = 6, BAR_PV_DONE = 8, BAR_O_EMPTY = 10, BAR_L_FULL = 12,
-       BAR_L_EMPTY = 14, BAR_RING = 16 };
+       BAR_L_EMPTY = 14, BAR_SCHED_FULL = 16, BAR_SCHED_EMPTY = 20, BAR_RING = 24 };
+constexpr int kSchedSlots = 4;
+constexpr int kSchedConsumers = 13;  // warps that read every item: MMA (1) + softmax (8) + epilogue (4)
 
 // Work item, 8 ints: {pos0, ntok0, ntok1, tok0 | r, kvh, q_off16, 0}.  The first int4 is all the softmax and MMA warps need.
 //   pos0: absolute position of the first token; ntok0/1: tokens of Q tile 0/1; tok0: index of the first token in [0,T);
@@ -103,7 +106,7 @@ template <int D>
 __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
     const __nv_bfloat16* __restrict__ q_roped, __nv_bfloat16* __restrict__ out,
     const __nv_bfloat16* __restrict__ k_pool, const __nv_bfloat16* __restrict__ v_pool,
-    const int32_t* __restrict__ tables, int max_blocks, const int4* __restrict__ work, int num_items,
+    const int32_t* __restrict__ tables, int max_blocks, int4* __restrict__ work, int num_items,
     int Hq, int Hkv, float scale_log2) {
     using L = Smem<D>;
     constexpr int NS = L::kStages;
@@ -118,6 +121,22 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
     const int tpt = kTileM / g;          // tokens per Q tile
     const int R = tpt * g;               // rows of a full Q tile
 
+    // Dynamic schedule: work[0].x is a counter (zeroed by the host with the list upload), items follow from work + 2.
+    // The loader warp claims items with atomicAdd and publishes each descriptor through a small smem ring; every other
+    // warp reads item #n from slot n % kSchedSlots (an item with ntok0 == 0 ends the stream).
+    const int4* items = work + 2;
+    auto get_item = [&](uint32_t n, bool full) {
+        const uint32_t slot = n % kSchedSlots;
+        ptx::mbar_wait(bar(BAR_SCHED_FULL + slot), (n / kSchedSlots) & 1u);
+        const int4* p = reinterpret_cast<const int4*>(smem + L::kSched + slot * 32);
+        const int4 a = p[0];
+        int4 b = make_int4(0, 0, 0, 0);
+        if (full) b = p[1];
+        __syncwarp();
+        if (lane == 0) ptx::mbar_arrive(bar(BAR_SCHED_EMPTY + slot));
+        return Item{a.x, a.y, a.z, a.w, b.x, b.y, b.z};
+    };
+
     if (threadIdx.x == 0) {
         for (int w = 0; w < 2; ++w) {
             ptx::mbar_init(bar(BAR_Q_FULL + w), 1);
@@ -128,6 +147,10 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
             ptx::mbar_init(bar(BAR_O_EMPTY + w), 128);
             ptx::mbar_init(bar(BAR_L_FULL + w), 128);
             ptx::mbar_init(bar(BAR_L_EMPTY + w), 128);
+        }
+        for (int s = 0; s < kSchedSlots; ++s) {
+            ptx::mbar_init(bar(BAR_SCHED_FULL + s), 1);
+            ptx::mbar_init(bar(BAR_SCHED_EMPTY + s), kSchedConsumers);
         }
         for (int s = 0; s < 2 * NS; ++s) ptx::mbar_init(bar(BAR_RING + s), 1);
         ptx::fence_mbar_init();
@@ -145,12 +168,35 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
             // Ring order per item: K(0) V(0) K(1) V(1) ...; the item's two Q tiles are loaded after K(0), V(0) so that
             // the MMA warp can chain QK(0) of this item right behind the last PV of the previous one.
             constexpr uint32_t kBlockBytes = 16 * D * 2;
-            uint32_t it = 0, qcnt0 = 0, qcnt1 = 0;
-            Item nxt = load_item(work, blockIdx.x);
-            for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
-                const Item w = nxt;
-                const bool has_next = idx + (int)gridDim.x < num_items;
-                if (has_next) nxt = load_item(work, idx + gridDim.x);
+            uint32_t it = 0, qcnt0 = 0, qcnt1 = 0, n_item = 0;
+            int* counter = reinterpret_cast<int*>(work);
+            auto claim = [&]() {                          // lane 0 holds the claimed index
+                int i = 0;
+                if (lane == 0) i = atomicAdd(counter, 1);
+                return i;
+            };
+            auto publish = [&](const Item& x, uint32_t n) {
+                const uint32_t slot = n % kSchedSlots;
+                ptx::mbar_wait(bar(BAR_SCHED_EMPTY + slot), ((n / kSchedSlots) & 1u) ^ 1u);
+                if (lane == 0) {
+                    int4* p = reinterpret_cast<int4*>(smem + L::kSched + slot * 32);
+                    p[0] = make_int4(x.pos0, x.ntok0, x.ntok1, x.tok0);
+                    p[1] = make_int4(x.r, x.kvh, x.q_off16, 0);
+                    ptx::mbar_arrive(bar(BAR_SCHED_FULL + slot));      // release: the stores above are visible to waiters
+                }
+                __syncwarp();
+            };
+            const Item kEnd{0, 0, 0, 0, 0, 0, 0};
+            int idx = __shfl_sync(0xffffffffu, claim(), 0);
+            Item w = idx < num_items ? load_item(items, idx) : kEnd;
+            publish(w, 0);
+            int idx_next = __shfl_sync(0xffffffffu, claim(), 0);
+            for (; w.ntok0 > 0; ++n_item) {
+                // next item: descriptor load and the claim after it are issued now and consumed after this item's first loads
+                const bool has_next = idx_next < num_items;
+                Item nxt = kEnd;
+                if (has_next) nxt = load_item(items, idx_next);
+                const int claimed = claim();
                 const int rows0 = w.ntok0 * g, rows1 = w.ntok1 * g;
                 const int nkv = w.pos0 + w.ntok0 + w.ntok1;
                 const int nt = tiles_for(nkv);
@@ -209,6 +255,8 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                                           (uint32_t)rows1 * 128u, bar(BAR_Q_FULL + 1));
                     }
                 }
+                publish(nxt, n_item + 1);
+                idx_next = __shfl_sync(0xffffffffu, claimed, 0);
                 if (has_next && lane == 0)   // pull the next item's Q tiles into L2 while this item computes
                     ptx::bulk_prefetch_l2(reinterpret_cast<const char*>(q_roped) + (size_t)nxt.q_off16 * 16,
                                           (uint32_t)((nxt.ntok0 + nxt.ntok1) * g * D * 2));
@@ -217,6 +265,7 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                     blk_next = j + 1 < nt ? load_ids(j + 1) : 0;
                     load_kv(j, blk);
                 }
+                w = nxt;
             }
         } else if (warp == 12) {
             // ================================ MMA issuer ================================
@@ -277,18 +326,18 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 if (ptx::elect_one()) issue_qk(w, slot_of(i0), n_w == 1);
                 __syncwarp();
             };
-            Item nxt = load_item_head(work, blockIdx.x);
-            if ((int)blockIdx.x < num_items) {
+            uint32_t n_item = 0;
+            Item w = get_item(0, false);
+            if (w.ntok0 > 0) {
                 wait_full(0);
-                open_tile(0, nxt, 0);
-                open_tile(1, nxt, 0);
+                open_tile(0, w, 0);
+                open_tile(1, w, 0);
                 if (ptx::elect_one()) release(0);
                 __syncwarp();
             }
-            for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
-                const Item w = nxt;
-                const bool has_next = idx + (int)gridDim.x < num_items;
-                if (has_next) nxt = load_item_head(work, idx + gridDim.x);
+            for (; w.ntok0 > 0; ++n_item) {
+                Item nxt{0, 0, 0, 0, 0, 0, 0};
+                bool has_next = false;
                 const int nkv0 = w.pos0 + w.ntok0, nkv1 = nkv0 + w.ntok1;
                 const int n0 = tiles_for(nkv0), n1 = w.ntok1 ? tiles_for(nkv1) : 0;
                 const int nt = n1 ? n1 : n0;
@@ -296,6 +345,10 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 for (int j = 0; j < nt; ++j) {
                     const uint32_t iv = it + 2 * j + 1, ikn = it + 2 * j + 2;   // ikn: K(j+1), or K(0) of the next item
                     const bool last_iter = j + 1 == nt;
+                    if (last_iter) {
+                        nxt = get_item(n_item + 1, false);
+                        has_next = nxt.ntok0 > 0;
+                    }
                     const int left = nkv - j * kTileN;
                     const int ksteps = left >= kTileN ? 8 : (left + 15) >> 4;   // skip 16-key steps with no valid key
                     wait_full(iv);
@@ -335,6 +388,7 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 it += 2u * (uint32_t)nt;
                 oitem0 += 1;
                 oitem1 += n1 ? 1u : 0u;
+                w = nxt;
             }
         }
         __syncwarp();
@@ -345,10 +399,9 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
         const uint32_t lane_base = ((uint32_t)((warp & 3) * 32)) << 16;
         const int tdiv = row / g, hh = row - tdiv * g;
         uint32_t cnt[2] = {0, 0}, litem[2] = {0, 0};
-        Item nxt = load_item(work, blockIdx.x);
-        for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
-            const Item w = nxt;
-            if (idx + (int)gridDim.x < num_items) nxt = load_item(work, idx + gridDim.x);
+        for (uint32_t n_item = 0;; ++n_item) {
+            const Item w = get_item(n_item, true);
+            if (w.ntok0 == 0) break;
 #pragma unroll
             for (int t = 0; t < 2; ++t) {
                 const int ntok = t ? w.ntok1 : w.ntok0;
@@ -394,10 +447,9 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
         const uint32_t tO = tmem + 256u + (uint32_t)wg * 128u + lane_base;
         const int tl = wg * tpt + row / g;                 // token of this row inside the item
         uint32_t cnt = 0, litem = 0;
-        Item nxt = load_item_head(work, blockIdx.x);
-        for (int idx = blockIdx.x; idx < num_items; idx += gridDim.x) {
-            const Item w = nxt;
-            if (idx + (int)gridDim.x < num_items) nxt = load_item_head(work, idx + gridDim.x);
+        for (uint32_t n_item = 0;; ++n_item) {
+            const Item w = get_item(n_item, false);
+            if (w.ntok0 == 0) break;
             const int ntok = wg ? w.ntok1 : w.ntok0;
             if (ntok == 0) continue;
             const int limit = w.pos0 + tl;                 // last visible key (inclusive); rows past the tile end are never stored
@@ -514,7 +566,7 @@ int64_t attn_count_tiles(const cw_config& cfg, const int32_t* h_cu, int32_t B) {
 }
 
 int64_t attn_work_ints(const cw_config& cfg, const int32_t* h_cu, int32_t B) {
-    return kWorkInts * attn_count_tiles(cfg, h_cu, B);
+    return kWorkInts * (attn_count_tiles(cfg, h_cu, B) + 1);   // + header (work counter)
 }
 
 // Item order: requests by descending work (longest first, so the tail of the launch is made of short items); inside
@@ -531,7 +583,7 @@ int64_t attn_build_schedule(const cw_config& cfg, const int32_t* h_cu, const int
         return s * (2 * c + s);                      // ~ number of (row, key) pairs
     };
     std::stable_sort(reqs.begin(), reqs.end(), [&](int a, int b) { return work_of(a) > work_of(b); });
-    work.clear();
+    work.assign(kWorkInts, 0);                        // header: work[0] = claim counter, zeroed with every upload
     for (int r : reqs) {
         const int s = h_cu[r + 1] - h_cu[r];
         const int npair = (s + 2 * tpt - 1) / (2 * tpt);
@@ -544,11 +596,11 @@ int64_t attn_build_schedule(const cw_config& cfg, const int32_t* h_cu, const int
                 work.insert(work.end(), item, item + kWorkInts);
             }
     }
-    return (int64_t)work.size() / kWorkInts;
+    return (int64_t)work.size() / kWorkInts - 1;
 }
 
 int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* tables, int32_t max_blocks,
-                        const int32_t* d_work, int64_t num_items, int num_sms, void* stream) {
+                        int32_t* d_work, int64_t num_items, int num_sms, void* stream) {
     if (num_items == 0) return 0;
     auto s = static_cast<cudaStream_t>(stream);
     const float scale_log2 = 1.4426950408889634f / sqrtf((float)cfg.head_dim);
@@ -561,7 +613,7 @@ int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, co
         if (e != cudaSuccess) return (int)e;                                                                        \
         prefill_attn_kernel<DD><<<grid, kThreads, Smem<DD>::kTotal, s>>>(                                           \
             (const __nv_bfloat16*)q_roped, (__nv_bfloat16*)out, (const __nv_bfloat16*)cfg.k_pool,                   \
-            (const __nv_bfloat16*)cfg.v_pool, tables, max_blocks, (const int4*)d_work, (int)num_items,              \
+            (const __nv_bfloat16*)cfg.v_pool, tables, max_blocks, (int4*)d_work, (int)num_items,              \
             cfg.num_q_heads, cfg.num_kv_heads, scale_log2);                                                         \
     } while (0)
     if (cfg.head_dim == 128) CW_LAUNCH_ATTN(128); else CW_LAUNCH_ATTN(64);
