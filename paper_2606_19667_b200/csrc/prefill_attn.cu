@@ -102,6 +102,10 @@ __device__ __forceinline__ int tiles_for(int nkv) { return (nkv + kTileN - 1) / 
 
 }  // namespace
 
+#ifdef CW_PROF   // experiments only: cycle counters per CTA
+__device__ unsigned long long cw_prof_buf[256][8];
+#endif
+
 template <int D>
 __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
     const __nv_bfloat16* __restrict__ q_roped, __nv_bfloat16* __restrict__ out,
@@ -457,8 +461,14 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
 
             float m_ref = -INFINITY, l_sum = 0.f;
             for (int j = 0; j < n_tiles; ++j, ++cnt) {
+#ifdef CW_PROF
+                const long long pt0 = clock64();
+#endif
                 ptx::mbar_wait(bar(BAR_S_FULL + wg), cnt & 1u);
                 ptx::tc_fence_after();
+#ifdef CW_PROF
+                const long long pt1 = clock64();
+#endif
 #ifdef CW_EXP_NOSOFTMAX   // timing experiment only (wrong results): the softmax group only hands the tile back
                 l_sum = 1.f;
                 ptx::tc_fence_before();
@@ -535,6 +545,13 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 ptx::tmem_st_wait();
                 ptx::tc_fence_before();
                 ptx::mbar_arrive(bar(BAR_P_FULL + wg));
+#ifdef CW_PROF
+                if (threadIdx.x == 0) {
+                    cw_prof_buf[blockIdx.x][1] += pt1 - pt0;            // wait for S
+                    cw_prof_buf[blockIdx.x][2] += clock64() - pt1;      // softmax compute until P_FULL arrive
+                    cw_prof_buf[blockIdx.x][7] += 1;
+                }
+#endif
             }
             // hand the row sum to the epilogue group and go on to the next item
             ptx::mbar_wait(bar(BAR_L_EMPTY + wg), (litem & 1u) ^ 1u);
@@ -622,3 +639,13 @@ int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, co
 }
 
 }  // namespace cw
+
+#ifdef CW_PROF
+extern "C" int cw_debug_prof(unsigned long long* out) {
+    cudaDeviceSynchronize();
+    int e = (int)cudaMemcpyFromSymbol(out, cw::cw_prof_buf, sizeof(cw::cw_prof_buf));
+    static unsigned long long zeros[256][8];
+    cudaMemcpyToSymbol(cw::cw_prof_buf, zeros, sizeof(zeros));
+    return e;
+}
+#endif
