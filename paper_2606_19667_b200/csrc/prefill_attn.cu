@@ -80,8 +80,12 @@ __device__ __forceinline__ Item load_item_head(const int4* __restrict__ work, in
 // exp2 on the FMA pipe for a share of the scores (the MUFU unit, 16 exp2 / clk / SM, is the softmax bottleneck):
 // 2^x = 2^round(x) * 2^f, f = x - round(x) in [-0.5, 0.5]; 2^f by a degree-3 polynomial (max rel. error 7.8e-5, P is
 // rounded to bf16 = 3.9e-3 afterwards); round(x) through the 1.5*2^23 magic constant, spliced into the exponent field.
-constexpr int kPolyPeriod = 4;       // of every kPolyPeriod score pairs ...
-constexpr int kPolyCount = 2;        // ... this many use the polynomial
+#ifndef CW_POLY_PERIOD
+#define CW_POLY_PERIOD 8
+#define CW_POLY_COUNT 1
+#endif
+constexpr int kPolyPeriod = CW_POLY_PERIOD;   // of every kPolyPeriod score pairs ...
+constexpr int kPolyCount = CW_POLY_COUNT;     // ... this many use the polynomial
 __device__ __forceinline__ float2 exp2_poly2(float2 x) {
     const float kMagic = 12582912.f;
     x.x = fmaxf(x.x, -125.f);
