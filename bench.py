@@ -289,6 +289,21 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+def max_over_ranks(value, dist, device):
+    """MAX of a scalar over all ranks (the only inter-rank exchange of the bench: timing plumbing, not data path)."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(units_per_rank, ms_max, world):
+    """whole-job throughput of `world` independent replicas ("replicas only"): all units processed / max time."""
+    return world * units_per_rank / (ms_max * 1e-3) / 1e12
+
+
 def timed(torch, fn, steps, dist):
     """barrier + sync, K steps, sync; device time by CUDA events on the launching (current) stream; max over ranks."""
     if dist is not None:
@@ -300,11 +315,8 @@ def timed(torch, fn, steps, dist):
         fn()
     e1.record()
     torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1)
+    ms = max_over_ranks(e0.elapsed_time(e1), dist, "cuda")
     if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
         dist.barrier()
     return ms
 
@@ -332,7 +344,7 @@ def run_ours(args):
         ms = timed(torch, lambda: wl.step(events), args.steps, dist)
     launches = wl.launches
     ms_step = ms / args.steps
-    value = world * wl.flops / (ms_step * 1e-3) / 1e12
+    value = aggregate_value(wl.flops, ms_step, world)
     app_ms = sum(e[0].elapsed_time(e[1]) for e in events) / args.steps       # per step, all waves
     attn_ms = sum(e[1].elapsed_time(e[2]) for e in events) / args.steps
     n_l = len(wl.waves)
@@ -345,7 +357,7 @@ def run_ours(args):
     wl.h2d = wl.d2h = 0
     e2e_steps = max(1, min(args.steps, args.e2e_steps))
     ms_e2e = timed(torch, wl.step_e2e, e2e_steps, dist) / e2e_steps
-    e2e_value = world * wl.flops / (ms_e2e * 1e-3) / 1e12
+    e2e_value = aggregate_value(wl.flops, ms_e2e, world)
 
     if rank != 0:
         if dist is not None:
