@@ -168,10 +168,13 @@ int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out,
  * (device int32 [ceil(n/16)]).  Used by tests and by callers that want the cached KV in a plain layout. */
 int cw_gather_kv(cw_ctx* ctx, const int32_t* d_block_table, int32_t n, void* k_out, void* v_out, void* stream);
 
-/* cw_prefill_host — the same path with HOST buffers (end-to-end entry point): copies q,k,v and the descriptors
- * to the caller-owned device workspace `d_ws` (cw_prefill_host_ws_bytes bytes), runs cw_append_kv +
- * cw_prefill_attn, copies out [T,Hq,D] back to host and synchronises the stream.  Host buffers should be pinned.
- * h_block_tables is [B, max_blocks_per_req]. */
+/* cw_prefill_host — the same path with HOST buffers (end-to-end entry point).  The batch is cut into up to 8 request
+ * chunks of about equal token count and pipelined: H2D of chunk i+1 (library-owned copy stream), cw_append_kv +
+ * cw_prefill_attn of chunk i (on `stream`, in request order), D2H of chunk i-1 (second copy stream); the call returns
+ * after everything has completed (both `stream` and the copy streams are synchronised).  q, k, v, out are staged in the
+ * caller-owned device workspace `d_ws` (cw_prefill_host_ws_bytes bytes).  Host buffers should be pinned (pageable
+ * memory works but serialises the copies).  h_block_tables is [B, max_blocks_per_req].  The two copy streams and their
+ * events are created on first use and destroyed by cw_destroy. */
 int64_t cw_prefill_host_ws_bytes(cw_ctx* ctx, int32_t B, int32_t T, int32_t max_blocks_per_req);
 int cw_prefill_host(cw_ctx* ctx, const void* h_q, const void* h_k, const void* h_v, void* h_out,
                     const int32_t* h_cu_seqlens_q, const int32_t* h_n_cached, const int32_t* h_block_tables,

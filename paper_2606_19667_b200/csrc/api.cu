@@ -107,6 +107,9 @@ int cw_create(const cw_config* cfg, cw_ctx** out) {
 
 void cw_destroy(cw_ctx* ctx) {
     if (!ctx) return;
+    for (void* e : ctx->events) cudaEventDestroy(static_cast<cudaEvent_t>(e));
+    if (ctx->copy_in_stream) cudaStreamDestroy(static_cast<cudaStream_t>(ctx->copy_in_stream));
+    if (ctx->copy_out_stream) cudaStreamDestroy(static_cast<cudaStream_t>(ctx->copy_out_stream));
     delete ctx->tree;
     delete ctx->blocks;
     delete ctx;
@@ -309,6 +312,7 @@ int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out, const int32_t* 
 
 // ---- host-buffer entry point ------------------------------------------------------------------------------
 namespace {
+constexpr int kHostChunks = 8;    // cw_prefill_host pipelines the batch in up to this many request chunks
 struct WsLayout {
     int64_t q, k, v, qr, out, cu, nc, tables, work, total;
 };
@@ -321,14 +325,14 @@ WsLayout ws_layout(const cw_config& c, int32_t B, int32_t T, int32_t max_blocks)
     w.v = o; o += align256(kb);
     w.qr = o; o += align256(qb);
     w.out = o; o += align256(qb);
-    w.cu = o; o += align256((int64_t)(B + 1) * 4);
+    w.cu = o; o += align256((int64_t)(B + 1 + kHostChunks) * 4);      // chunk-local prefix sums: (B_c + 1) ints per chunk
     w.nc = o; o += align256((int64_t)B * 4);
     w.tables = o; o += align256((int64_t)B * max_blocks * 4);
     // upper bound on tiles: every request may add one ragged tile per kv head
     const int g = c.num_q_heads / c.num_kv_heads;
     const int tpt2 = 2 * (128 / g);
     const int64_t max_items = (((int64_t)T + tpt2 - 1) / tpt2 + B) * c.num_kv_heads;
-    w.work = o; o += align256((max_items + 1) * 32);
+    w.work = o; o += align256((max_items + kHostChunks) * 32) + 256 * kHostChunks;   // one list (+ header) per chunk
     w.total = o;
     return w;
 }
@@ -347,27 +351,86 @@ int cw_prefill_host(cw_ctx* ctx, const void* h_q, const void* h_k, const void* h
     if (T == 0 || B == 0) return CW_OK;
     if (!h_q || !h_k || !h_v || !h_out || !h_cu || !h_nc || !h_tables || !d_ws)
         return fail(ctx, CW_ERR_INVALID, "cw_prefill_host: null pointer");
+    if (h_cu[0] != 0 || h_cu[B] != T) return fail(ctx, CW_ERR_INVALID, "cw_prefill_host: cu_seqlens_q does not span T");
     const cw_config& c = ctx->cfg;
     const WsLayout w = ws_layout(c, B, T, max_blocks);
     auto s = static_cast<cudaStream_t>(stream);
     char* ws = static_cast<char*>(d_ws);
-    const size_t qb = (size_t)T * c.num_q_heads * c.head_dim * 2, kb = (size_t)T * c.num_kv_heads * c.head_dim * 2;
-    cudaError_t e = cudaMemcpyAsync(ws + w.q, h_q, qb, cudaMemcpyHostToDevice, s);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(ws + w.k, h_k, kb, cudaMemcpyHostToDevice, s);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(ws + w.v, h_v, kb, cudaMemcpyHostToDevice, s);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(ws + w.cu, h_cu, (size_t)(B + 1) * 4, cudaMemcpyHostToDevice, s);
+    cudaError_t e = cudaSuccess;
+    // The batch is cut into request chunks of about equal token count and pipelined over three streams: H2D of chunk i+1
+    // (copy-in stream), RoPE + scatter and attention of chunk i (caller's stream, in request order: later requests may read
+    // blocks written by earlier ones of the same batch), D2H of chunk i-1 (copy-out stream).  PCIe is full duplex, so the
+    // end-to-end time approaches max(H2D, D2H) instead of their sum.
+    if (!ctx->copy_in_stream) {
+        cudaStream_t a = nullptr, b = nullptr;
+        e = cudaStreamCreateWithFlags(&a, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&b, cudaStreamNonBlocking);
+        if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_host (streams)");
+        ctx->copy_in_stream = a;
+        ctx->copy_out_stream = b;
+        for (int i = 0; i < 2 * kHostChunks + 1; ++i) {
+            cudaEvent_t ev;
+            e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+            if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_host (events)");
+            ctx->events.push_back(ev);
+        }
+    }
+    auto s_in = static_cast<cudaStream_t>(ctx->copy_in_stream), s_out = static_cast<cudaStream_t>(ctx->copy_out_stream);
+    auto ev = [&](int i) { return static_cast<cudaEvent_t>(ctx->events[(size_t)i]); };
+    // chunk boundaries (request indices) and chunk-local prefix sums
+    const int nch = std::min<int>(kHostChunks, B);
+    std::vector<int32_t> first((size_t)nch + 1, B), cu_local;
+    first[0] = 0;
+    for (int k = 1, r = 0; k < nch; ++k) {
+        const int64_t target = (int64_t)T * k / nch;
+        while (r < B && h_cu[r] < target) ++r;
+        first[(size_t)k] = std::max(r, first[(size_t)k - 1]);
+    }
+    std::vector<int64_t> cu_off((size_t)nch);
+    for (int k = 0; k < nch; ++k) {
+        cu_off[(size_t)k] = (int64_t)cu_local.size();
+        for (int r = first[(size_t)k]; r <= first[(size_t)k + 1]; ++r) cu_local.push_back(h_cu[r] - h_cu[first[(size_t)k]]);
+    }
+    // descriptors first (small), on the caller's stream; copies of activations wait for everything queued before us
+    e = cudaMemcpyAsync(ws + w.cu, cu_local.data(), cu_local.size() * 4, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(ws + w.nc, h_nc, (size_t)B * 4, cudaMemcpyHostToDevice, s);
     if (e == cudaSuccess) e = cudaMemcpyAsync(ws + w.tables, h_tables, (size_t)B * max_blocks * 4, cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_host (H2D)");
-    int rc = cw_append_kv(ctx, ws + w.q, ws + w.k, ws + w.v, ws + w.qr, (const int32_t*)(ws + w.cu),
-                          (const int32_t*)(ws + w.nc), (const int32_t*)(ws + w.tables), max_blocks, B, T, stream);
-    if (rc != CW_OK) return rc;
-    rc = cw_prefill_attn(ctx, ws + w.qr, ws + w.out, h_cu, h_nc, (const int32_t*)(ws + w.cu), (const int32_t*)(ws + w.nc),
-                         (const int32_t*)(ws + w.tables), max_blocks, B, T, (int32_t*)(ws + w.work), stream);
-    if (rc != CW_OK) return rc;
-    e = cudaMemcpyAsync(h_out, ws + w.out, qb, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaEventRecord(ev(2 * kHostChunks), s);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s_in, ev(2 * kHostChunks), 0);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s_out, ev(2 * kHostChunks), 0);
+    if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_host (descriptors)");
+    const size_t qrow = (size_t)c.num_q_heads * c.head_dim * 2, krow = (size_t)c.num_kv_heads * c.head_dim * 2;
+    int64_t work_off = 0;
+    for (int k = 0; k < nch; ++k) {
+        const int r0 = first[(size_t)k], r1 = first[(size_t)k + 1], Bc = r1 - r0;
+        const int64_t t0 = h_cu[r0], Tc = h_cu[r1] - t0;
+        if (Bc == 0 || Tc == 0) continue;
+        e = cudaMemcpyAsync(ws + w.q + t0 * qrow, (const char*)h_q + t0 * qrow, Tc * qrow, cudaMemcpyHostToDevice, s_in);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(ws + w.k + t0 * krow, (const char*)h_k + t0 * krow, Tc * krow, cudaMemcpyHostToDevice, s_in);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(ws + w.v + t0 * krow, (const char*)h_v + t0 * krow, Tc * krow, cudaMemcpyHostToDevice, s_in);
+        if (e == cudaSuccess) e = cudaEventRecord(ev(k), s_in);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s, ev(k), 0);
+        if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_host (H2D)");
+        const int32_t* d_cu = (const int32_t*)(ws + w.cu) + cu_off[(size_t)k];
+        const int32_t* d_nc = (const int32_t*)(ws + w.nc) + r0;
+        const int32_t* d_tab = (const int32_t*)(ws + w.tables) + (size_t)r0 * max_blocks;
+        const int32_t* hc = cu_local.data() + cu_off[(size_t)k];
+        int rc = cw_append_kv(ctx, ws + w.q + t0 * qrow, ws + w.k + t0 * krow, ws + w.v + t0 * krow, ws + w.qr + t0 * qrow, d_cu, d_nc,
+                              d_tab, max_blocks, Bc, (int32_t)Tc, stream);
+        if (rc != CW_OK) return rc;
+        int32_t* d_work = (int32_t*)(ws + w.work) + work_off;
+        rc = cw_prefill_attn(ctx, ws + w.qr + t0 * qrow, ws + w.out + t0 * qrow, hc, h_nc + r0, d_cu, d_nc, d_tab, max_blocks, Bc,
+                             (int32_t)Tc, d_work, stream);
+        if (rc != CW_OK) return rc;
+        work_off += (cw::attn_work_ints(c, hc, Bc) + 63) / 64 * 64;
+        e = cudaEventRecord(ev(kHostChunks + k), s);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s_out, ev(kHostChunks + k), 0);
+        if (e == cudaSuccess) e = cudaMemcpyAsync((char*)h_out + t0 * qrow, ws + w.out + t0 * qrow, Tc * qrow, cudaMemcpyDeviceToHost, s_out);
+        if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_host (D2H)");
+    }
+    e = cudaStreamSynchronize(s_out);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_host (D2H)");
+    if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_host (sync)");
     return CW_OK;
 }
 

@@ -98,6 +98,10 @@ struct cw_ctx {
     std::string last_error;
     bool host_only;
     int num_sms;
+    // cw_prefill_host pipeline: copy streams and per-chunk events (created on first use, destroyed with the context)
+    void* copy_in_stream = nullptr;
+    void* copy_out_stream = nullptr;
+    std::vector<void*> events;
 };
 
 // kernel launchers (defined in the .cu files); return cudaError_t as int

@@ -234,3 +234,25 @@ def test_trace_cfg2_first_requests_all_rows(dev):
         assert_close_attn(a.out, o.out, f"cfg2 r={a.r} c={a.n_cached}")
         hits += a.n_cached
     assert hits > 0, "the greedy arm must reuse some prefix on config 2"
+
+
+def test_prefill_host_equals_device_path(dev):
+    """cw_prefill_host (pinned host buffers, chunked H2D / compute / D2H pipeline) gives bit-identical outputs to the
+    device-buffer calls, and matches the oracle."""
+    cs, ss = [0, 64, 0, 256, 16, 0, 128, 0, 32, 0], [130, 200, 1, 48, 300, 77, 64, 129, 500, 31]
+    b = Batch(dev, 32, 8, 128, cs, ss, seed=7)
+    _, out_dev, cu = b.run()
+    b2 = Batch(dev, 32, 8, 128, cs, ss, seed=7)
+    b2._append([0] * b2.B, b2.cs)                      # cached prefixes
+    cat = lambda xs: np.concatenate([x[c:] for x, c in zip(xs, b2.cs)], axis=0)
+    hq, hk, hv = (torch.from_numpy(cat(x).view(np.int16)).view(torch.bfloat16).pin_memory() for x in (b2.q, b2.k, b2.v))
+    hout = torch.empty_like(hq).pin_memory()
+    T = int(cu[-1])
+    ws = torch.empty(b2.ctx.cw_prefill_host_ws_bytes(b2.B, T, b2.max_blocks), dtype=torch.uint8, device=dev)
+    for _ in range(2):                                   # second call reuses the streams / events
+        hout.zero_()
+        b2.ctx.cw_prefill_host(hq, hk, hv, hout, cu, np.asarray(cs, np.int32), b2.tables, b2.max_blocks, b2.B, T, ws)
+        got = hout.view(torch.int16).numpy().view(np.uint16)
+        assert np.array_equal(got, out_dev)
+    for r in range(b.B):
+        assert_close_attn(out_dev[cu[r]:cu[r + 1]], b.oracle(r), f"r={r}")
