@@ -110,7 +110,7 @@ class Workload:
     """One configuration, one strategy: seeded trace, resident inputs, and the step function."""
     RING = 4
 
-    def __init__(self, cfg_id, strategy, device, want_e2e=True):
+    def __init__(self, cfg_id, strategy, device, want_e2e=True, device_inputs=False):
         import torch
         from paper_2606_19667_b200.engine import admit_waves, make_context
         self.torch, self.device, self.strategy = torch, device, strategy
@@ -127,7 +127,17 @@ class Workload:
         self.max_blocks = cfg.blocks_per_req
         Bmax = max(w.B for w in self.waves)
         self.inputs, self.host_inputs = [], []
-        for w in self.waves:
+        for wi, w in enumerate(self.waves):
+            if device_inputs:
+                # timing-only runs of the large configs / the sweep: seeded N(0,1) bf16 drawn on the device (the values do
+                # not change the work; parity at these shapes is covered by tests/test_gpu_full_size.py with tracegen inputs)
+                g = torch.Generator(device=device)
+                g.manual_seed(cfg.seed * 1000 + wi)
+                dq, dk, dv = (torch.randn(w.T, h, cfg.D, device=device, dtype=torch.bfloat16, generator=g)
+                              for h in (cfg.Hq, cfg.Hkv, cfg.Hkv))
+                work = torch.empty(max(4, self.ctx.cw_attn_work_ints(w.cu)), dtype=torch.int32, device=device)
+                self.inputs.append((dq, dk, dv, torch.empty_like(dq), torch.empty_like(dq), work))
+                continue
             rows = tracegen.batch_suffix_qkv(trace, w.items, threads=os.cpu_count() or 8)
             qkv = [torch.from_numpy(x.view(np.int16)).view(torch.bfloat16) for x in tracegen.split_qkv(cfg, rows)]
             if want_e2e:
@@ -333,7 +343,7 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(device))
     pk = peaks()
-    wl = Workload(args.config, "greedy", device)
+    wl = Workload(args.config, "greedy", device, want_e2e=not args.device_inputs, device_inputs=args.device_inputs)
     cfg = wl.cfg
 
     for _ in range(args.warmup):
@@ -352,12 +362,14 @@ def run_ours(args):
     app_gbs = append_bytes(cfg, wl.T) / (app_ms * 1e-3) / 1e9
 
     # end to end: host buffers, H2D/D2H inside the timed region
-    for _ in range(max(1, args.warmup // 2)):
-        wl.step_e2e()
-    wl.h2d = wl.d2h = 0
-    e2e_steps = max(1, min(args.steps, args.e2e_steps))
-    ms_e2e = timed(torch, wl.step_e2e, e2e_steps, dist) / e2e_steps
-    e2e_value = aggregate_value(wl.flops, ms_e2e, world)
+    e2e_steps, ms_e2e, e2e_value = 0, None, None
+    if not args.device_inputs:
+        for _ in range(max(1, args.warmup // 2)):
+            wl.step_e2e()
+        wl.h2d = wl.d2h = 0
+        e2e_steps = max(1, min(args.steps, args.e2e_steps))
+        ms_e2e = timed(torch, wl.step_e2e, e2e_steps, dist) / e2e_steps
+        e2e_value = aggregate_value(wl.flops, ms_e2e, world)
 
     if rank != 0:
         if dist is not None:
@@ -368,7 +380,7 @@ def run_ours(args):
                           "hit_blocks": wl.hit_blocks, "attn_flops": wl.flops}}
     if not args.skip_retrieval:
         del wl.host_inputs, wl.ws
-        wr = Workload(args.config, "retrieval", device, want_e2e=False)
+        wr = Workload(args.config, "retrieval", device, want_e2e=False, device_inputs=args.device_inputs)
         for _ in range(args.warmup):
             wr.step()
         ev = []
@@ -391,7 +403,7 @@ def run_ours(args):
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
-            "data": "synthetic",
+            "data": "synthetic" + (" (timing-only activations drawn on the device)" if args.device_inputs else ""),
             "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({cfg.name})", "requests": cfg.n_req,
                        "prompt_tokens": cfg.n, "heads": f"{cfg.Hq}q/{cfg.Hkv}kv x {cfg.D}", "pool_blocks": cfg.NB,
                        "admission": f"one varlen wave per launch ({n_l} wave(s)), eager block registration",
@@ -399,8 +411,8 @@ def run_ours(args):
                        "l2": "inputs larger than L2 (q,k,v,pool >> 126 MB per step); no explicit flush"},
             "pct_of_bf16_peak": 100.0 * value / world / pk["bf16"],
             "clocks": clk.summary(),
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": wl.h2d // e2e_steps,
-                    "d2h_bytes_per_step": wl.d2h // e2e_steps, "ms_per_step": ms_e2e, "steps": e2e_steps},
+            "e2e": ({"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": wl.h2d // e2e_steps,
+                     "d2h_bytes_per_step": wl.d2h // e2e_steps, "ms_per_step": ms_e2e, "steps": e2e_steps} if e2e_steps else None),
             "gpu_launches": launches,
             "roofline": {"kernel": "prefill_attn_kernel", "bound": "tensor", "achieved": attn_tflops, "peak": pk["bf16"],
                          "unit": "TFLOP/s", "frac": attn_tflops / pk["bf16"], "traffic": traffic_from_profile("prefill_attn_kernel"),
@@ -416,6 +428,37 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """BASELINE.json configs[2]: adjacent-overlap x top-k sweep at the 8B shapes, both orderings; per cell: hit blocks,
+    suffix tokens, attention flops and prefill ms (append + attention, one wave per launch).  Timing-only inputs."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback")
+    device = "cuda:0"
+    cells = []
+    for k in (3, 5, 10):
+        for ov in (0, 30, 60, 90):
+            cell = {"k": k, "overlap_pct": ov}
+            for arm in ("retrieval", "greedy"):
+                wl = Workload(tracegen.config3(k, ov), arm, device, want_e2e=False, device_inputs=True)
+                for _ in range(max(3, args.warmup)):
+                    wl.step()
+                ev = []
+                timed(torch, lambda: wl.step(ev), args.steps, None)
+                app = sum(e[0].elapsed_time(e[1]) for e in ev) / args.steps
+                att = sum(e[1].elapsed_time(e[2]) for e in ev) / args.steps
+                cell[arm] = {"hit_blocks": wl.hit_blocks, "suffix_tokens": wl.T, "attn_flops": wl.flops, "waves": len(wl.waves),
+                             "prefill_ms": app + att, "append_ms": app, "attn_ms": att,
+                             "attn_tflops": wl.flops / (att * 1e-3) / 1e12}
+                del wl
+                torch.cuda.empty_cache()
+            cell["flops_ratio"] = cell["greedy"]["attn_flops"] / cell["retrieval"]["attn_flops"]
+            cell["ms_ratio"] = cell["greedy"]["prefill_ms"] / cell["retrieval"]["prefill_ms"]
+            cells.append(cell)
+            print(json.dumps(cell), flush=True)
+    return cells
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -426,11 +469,15 @@ def main():
     ap.add_argument("--oracle-requests", type=int, default=None, help="requests in the oracle's bounded sample")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--skip-retrieval", action="store_true")
+    ap.add_argument("--device-inputs", action="store_true", help="timing-only: draw q,k,v on the device (no e2e leg)")
+    ap.add_argument("--sweep", action="store_true", help="overlap x top-k sweep (BASELINE.json configs[2]), one JSON line per cell")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.oracle_requests is None:
         args.oracle_requests = {1: 4, 2: 16 if args.impl == "ours" else 4, 4: 1, 5: 1}[args.config]
-    if args.impl == "reference":
+    if args.sweep:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
