@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(128) append_kv_kernel(
         const int tib = p & 15;
         const int prow = p < max_position ? p : max_position - 1;
         const float4* cs_row = reinterpret_cast<const float4*>(rope_table + (size_t)prow * D);
-        for (int u = threadIdx.x; u < units; u += blockDim.x) {
+        for (int u = threadIdx.x; u < units; u += 128) {
             if (u < uq) {
                 const int h = u / CPH, c = u % CPH;
                 const size_t off = ((size_t)tok * Hq + h) * D + c * 8;
@@ -119,16 +119,8 @@ int launch_append_kv(const cw_config& cfg, const void* q, const void* k, const v
     if (T == 0) return 0;
     int grid = T < 148 * 16 ? T : 148 * 16;
     auto s = static_cast<cudaStream_t>(stream);
-    // threads per CTA: the multiple of 32 (<= 128) that wastes the fewest lanes on the token's units
-    // (8B: 384 units = 3 x 128; 70B: 640 = 5 x 128; Qwen2.5-7B: 288 = 3 x 96)
-    const int units = (cfg.num_q_heads + 2 * cfg.num_kv_heads) * (cfg.head_dim / 16);
-    int threads = 128, best_waste = 1 << 30;
-    for (int t = 128; t >= 64; t -= 32) {
-        const int waste = (units + t - 1) / t * t - units;
-        if (waste < best_waste) { best_waste = waste; threads = t; }
-    }
 #define CW_LAUNCH_APPEND(DD)                                                                                    \
-    append_kv_kernel<DD><<<grid, threads, 0, s>>>(                                                                  \
+    append_kv_kernel<DD><<<grid, 128, 0, s>>>(                                                                  \
         (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, (__nv_bfloat16*)q_roped,     \
         (__nv_bfloat16*)cfg.k_pool, (__nv_bfloat16*)cfg.v_pool, (const float*)cfg.rope_table, cu, ncached,      \
         tables, max_blocks, B, T, cfg.num_q_heads, cfg.num_kv_heads, cfg.max_position)

@@ -36,6 +36,7 @@ constexpr int kTileN = 128;          // keys per KV tile (8 pool blocks)
 constexpr int kThreads = 512;
 constexpr int kWorkInts = 8;         // ints per work item
 constexpr float kRescaleThreshold = 8.0f;   // log2 units
+constexpr float kSpecLimit = 65536.f;       // bound on a row sum taken against a stale reference maximum
 
 template <int D>
 struct Smem {
@@ -479,55 +480,71 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 ptx::mbar_arrive(bar(BAR_P_FULL + wg));
                 continue;
 #endif
+                // Speculative path for j > 0: skip the max pass and take exp2 against the current reference maximum; the row
+                // sum then bounds every P entry (P <= sum <= 2^16 is exact in fp32/bf16 — softmax does not depend on the
+                // reference).  If any row of the warp exceeds the bound (or holds a NaN), the warp redoes the tile the
+                // exact way: tile maximum, lazy rescale.  S stays intact in TMEM until P is stored, so it is re-read.
                 uint32_t sv[4][32];
+                float alpha = 1.f;
+                bool grow = false;
+                bool spec = j > 0;
+                for (;;) {
 #pragma unroll
-                for (int i = 0; i < 4; ++i) ptx::tmem_ld32(tS + i * 32, sv[i]);
-                ptx::tmem_ld_wait();
+                    for (int i = 0; i < 4; ++i) ptx::tmem_ld32(tS + i * 32, sv[i]);
+                    ptx::tmem_ld_wait();
 
-                const int kbase = j * kTileN;
-                if (kbase + kTileN - 1 > limit) {
+                    const int kbase = j * kTileN;
+                    if (kbase + kTileN - 1 > limit) {
+#pragma unroll
+                        for (int i = 0; i < 4; ++i)
+#pragma unroll
+                            for (int e = 0; e < 32; ++e)
+                                if (kbase + i * 32 + e > limit) sv[i][e] = 0xFF800000u;   // -inf
+                    }
+                    if (!spec) {
+                        float tm[4];
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            float a = fmaxf(__uint_as_float(sv[i][0]), __uint_as_float(sv[i][1]));
+                            float b = fmaxf(__uint_as_float(sv[i][2]), __uint_as_float(sv[i][3]));
+#pragma unroll
+                            for (int e = 4; e < 32; e += 4) {
+                                a = fmaxf(a, fmaxf(__uint_as_float(sv[i][e]), __uint_as_float(sv[i][e + 1])));
+                                b = fmaxf(b, fmaxf(__uint_as_float(sv[i][e + 2]), __uint_as_float(sv[i][e + 3])));
+                            }
+                            tm[i] = fmaxf(a, b);
+                        }
+                        const float tmax = fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3]));
+                        // lazy rescale decision (per row); the TMEM round trip below is made warp-uniform
+                        grow = (tmax - m_ref) * scale_log2 > kRescaleThreshold;   // true on the first tile (m_ref = -inf)
+                        if (grow) {
+                            alpha = ptx::ex2((m_ref - tmax) * scale_log2);        // 0 on the first tile
+                            m_ref = tmax;
+                        }
+                    }
+                    const float mneg = -m_ref * scale_log2;
+                    const float2 sc2 = make_float2(scale_log2, scale_log2), mn2 = make_float2(mneg, mneg);
+                    float2 ps[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
 #pragma unroll
                     for (int i = 0; i < 4; ++i)
 #pragma unroll
-                        for (int e = 0; e < 32; ++e)
-                            if (kbase + i * 32 + e > limit) sv[i][e] = 0xFF800000u;   // -inf
-                }
-                float tm[4];
-#pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    float a = fmaxf(__uint_as_float(sv[i][0]), __uint_as_float(sv[i][1]));
-                    float b = fmaxf(__uint_as_float(sv[i][2]), __uint_as_float(sv[i][3]));
-#pragma unroll
-                    for (int e = 4; e < 32; e += 4) {
-                        a = fmaxf(a, fmaxf(__uint_as_float(sv[i][e]), __uint_as_float(sv[i][e + 1])));
-                        b = fmaxf(b, fmaxf(__uint_as_float(sv[i][e + 2]), __uint_as_float(sv[i][e + 3])));
+                        for (int e = 0; e < 32; e += 2) {
+                            // packed fp32x2 FMA / ADD (sm_100): one instruction per pair of scores
+                            const float2 x = __ffma2_rn(make_float2(__uint_as_float(sv[i][e]), __uint_as_float(sv[i][e + 1])), sc2, mn2);
+                            float2 p;
+                            if (((e >> 1) % kPolyPeriod) < kPolyCount) p = exp2_poly2(x);        // FMA pipe
+                            else p = make_float2(ptx::ex2(x.x), ptx::ex2(x.y));                  // MUFU (16 / clk / SM)
+                            ps[(e >> 1) & 3] = __fadd2_rn(ps[(e >> 1) & 3], p);
+                            sv[i >> 1][(i & 1) * 16 + (e >> 1)] = ptx::pack_bf16x2(p.x, p.y);   // packed P: 64 registers
+                        }
+                    const float psum = ((ps[0].x + ps[0].y) + (ps[1].x + ps[1].y)) + ((ps[2].x + ps[2].y) + (ps[3].x + ps[3].y));
+                    if (spec && __any_sync(0xffffffffu, !(psum <= kSpecLimit))) {
+                        spec = false;
+                        continue;
                     }
-                    tm[i] = fmaxf(a, b);
+                    l_sum = l_sum * alpha + psum;
+                    break;
                 }
-                const float tmax = fmaxf(fmaxf(tm[0], tm[1]), fmaxf(tm[2], tm[3]));
-                // lazy rescale decision (per row); the TMEM round trip below is made warp-uniform
-                float alpha = 1.f;
-                const bool grow = (tmax - m_ref) * scale_log2 > kRescaleThreshold;   // true on the first tile (m_ref = -inf)
-                if (grow) {
-                    alpha = ptx::ex2((m_ref - tmax) * scale_log2);                   // 0 on the first tile
-                    m_ref = tmax;
-                }
-                const float mneg = -m_ref * scale_log2;
-                const float2 sc2 = make_float2(scale_log2, scale_log2), mn2 = make_float2(mneg, mneg);
-                float2 ps[4] = {make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f), make_float2(0.f, 0.f)};
-#pragma unroll
-                for (int i = 0; i < 4; ++i)
-#pragma unroll
-                    for (int e = 0; e < 32; e += 2) {
-                        // packed fp32x2 FMA / ADD (sm_100): one instruction per pair of scores
-                        const float2 x = __ffma2_rn(make_float2(__uint_as_float(sv[i][e]), __uint_as_float(sv[i][e + 1])), sc2, mn2);
-                        float2 p;
-                        if (((e >> 1) % kPolyPeriod) < kPolyCount) p = exp2_poly2(x);        // FMA pipe
-                        else p = make_float2(ptx::ex2(x.x), ptx::ex2(x.y));                  // MUFU (16 / clk / SM)
-                        ps[(e >> 1) & 3] = __fadd2_rn(ps[(e >> 1) & 3], p);
-                        sv[i >> 1][(i & 1) * 16 + (e >> 1)] = ptx::pack_bf16x2(p.x, p.y);   // packed P: 64 registers
-                    }
-                l_sum = l_sum * alpha + (((ps[0].x + ps[0].y) + (ps[1].x + ps[1].y)) + ((ps[2].x + ps[2].y) + (ps[3].x + ps[3].y)));
 
                 if (j > 0 && __any_sync(0xffffffffu, grow)) {
                     // O_w holds the sum up to tile j-1: S_FULL(j) was committed after PV(j-1), so it is complete

@@ -256,3 +256,28 @@ def test_prefill_host_equals_device_path(dev):
         assert np.array_equal(got, out_dev)
     for r in range(b.B):
         assert_close_attn(out_dev[cu[r]:cu[r + 1]], b.oracle(r), f"r={r}")
+
+
+def test_attention_growing_maximum_takes_the_exact_path(dev):
+    """Scores that grow by far more than the lazy-rescale threshold from one KV tile to the next (keys scaled up along
+    the sequence) force the speculative stale-maximum path to fall back to the exact one and rescale O.  With logits this
+    large the bf16 rounding of the roped Q/K alone moves the outputs by more than 2e-2, so the reference here is the
+    oracle's attention applied to the oracle's roped Q/K rounded to bf16 (what the pool holds); the plain oracle is
+    still checked in relative L2."""
+    b = Batch(dev, 8, 2, 128, cs=[0, 128], ss=[700, 400], seed=11)
+    for r in range(b.B):
+        n = b.ns[r]
+        ramp = (1.0 + 7.0 * (np.arange(n) // 128) / max(1, (n - 1) // 128)).astype(np.float32)      # x1 .. x8 per KV tile
+        k = tracegen.bf16_bits_to_f64(b.k[r]).astype(np.float32) * ramp[:, None, None]
+        b.k[r] = tracegen.f32_to_bf16_bits(k)
+    _, out_bits, cu = b.run()
+    f, rnd = tracegen.bf16_bits_to_f64, lambda x: tracegen.bf16_bits_to_f64(tracegen.f32_to_bf16_bits(x.astype(np.float32)))
+    for r in range(b.B):
+        n, c = b.ns[r], b.cs[r]
+        pos = np.arange(n)
+        q_r, k_r = rnd(oattn.rope(f(b.q[r]), pos, b.theta)), rnd(oattn.rope(f(b.k[r]), pos, b.theta))
+        ref_q = oattn.attention_rows(q_r[c:], k_r, f(b.v[r]), pos[c:])
+        assert_close_attn(out_bits[cu[r]:cu[r + 1]], ref_q, f"r={r} (bf16-rounded roped Q/K)")
+        got = f(out_bits[cu[r]:cu[r + 1]])
+        ref = b.oracle(r)
+        assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= REL_L2
