@@ -110,7 +110,7 @@ class Workload:
     """One configuration, one strategy: seeded trace, resident inputs, and the step function."""
     RING = 4
 
-    def __init__(self, cfg_id, strategy, device, want_e2e=True, device_inputs=False):
+    def __init__(self, cfg_id, strategy, device, want_e2e=True, device_inputs=False, sequential=False):
         import torch
         from paper_2606_19667_b200.engine import admit_waves, make_context
         self.torch, self.device, self.strategy = torch, device, strategy
@@ -119,7 +119,8 @@ class Workload:
         self.ctx = make_context(cfg, device)
         self.doc_ids = np.asarray(trace.retrieval, dtype=np.int64)
         # dry admission (host only) fixes the wave boundaries and suffix descriptors; every step repeats it for real
-        self.waves = admit_waves(self.ctx, trace, strategy)
+        self.sequential = sequential          # one request per wave (per-request launches) instead of as many as fit
+        self.waves = admit_waves(self.ctx, trace, strategy, force_waves=not sequential)
         self.ctx.cw_reset()
         self.flops = sum(attention_flops(cfg, w.nc) for w in self.waves)
         self.T = sum(w.T for w in self.waves)
@@ -175,7 +176,7 @@ class Workload:
         self.slot = (self.slot + 1) % self.RING
         if st["event"] is not None:
             st["event"].synchronize()
-        hi = lo + self.Bmax + 1
+        hi = lo + (expect.B if self.sequential else self.Bmax + 1)
         a = self.ctx.cw_admit_batch(self.doc_ids[lo:hi], self.strategy == "greedy", self.trace.doc_tokens,
                                     self.queries[lo:hi], self.max_blocks, out=st["np"])
         if a["admitted"] != expect.B:
@@ -392,6 +393,16 @@ def run_ours(args):
         prefill["ratio_measured"] = prefill["greedy"]["ms"] / prefill["retrieval"]["ms"]
         prefill["ratio_predicted_by_flops"] = wl.flops / wr.flops
         del wr
+        if cfg.admission == "sequential":
+            # the honest per-request figure: every request admitted, launched (2 kernels) and released
+            # on its own — launch-bound on this shape (one request is 5-15 us of tensor work)
+            ws = Workload(args.config, "greedy", device, want_e2e=False, device_inputs=True, sequential=True)
+            for _ in range(args.warmup):
+                ws.step()
+            s_ms = timed(torch, ws.step, args.steps, None) / args.steps
+            prefill["per_request_launches"] = {"ms_per_trace": s_ms, "launches": 2 * len(ws.waves), "attn_flops": ws.flops,
+                                               "value_tflops": ws.flops / (s_ms * 1e-3) / 1e12}
+            del ws
 
     cpu = None
     if world == 1 or rank == 0:
