@@ -53,8 +53,8 @@ __device__ __forceinline__ int pool_chunk_offset(int t, int d) {
     return (t >> 3) * (8 * D) + (d >> 6) * 512 + (t & 7) * 64 + ((((d & 63) >> 3) ^ (t & 7)) << 3);
 }
 
-template <int D>
-__global__ void __launch_bounds__(128) append_kv_kernel(
+template <int D, int THREADS>
+__global__ void __launch_bounds__(THREADS) append_kv_kernel(
     const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ k, const __nv_bfloat16* __restrict__ v,
     __nv_bfloat16* __restrict__ q_roped, __nv_bfloat16* __restrict__ k_pool, __nv_bfloat16* __restrict__ v_pool,
     const float* __restrict__ rope_table, const int32_t* __restrict__ cu, const int32_t* __restrict__ ncached,
@@ -82,7 +82,7 @@ __global__ void __launch_bounds__(128) append_kv_kernel(
         const int tib = p & 15;
         const int prow = p < max_position ? p : max_position - 1;
         const float4* cs_row = reinterpret_cast<const float4*>(rope_table + (size_t)prow * D);
-        for (int u = threadIdx.x; u < units; u += 128) {
+        for (int u = threadIdx.x; u < units; u += THREADS) {
             if (u < uq) {
                 const int h = u / CPH, c = u % CPH;
                 const size_t off = ((size_t)tok * Hq + h) * D + c * 8;
@@ -117,14 +117,30 @@ int launch_append_kv(const cw_config& cfg, const void* q, const void* k, const v
                      const int32_t* cu, const int32_t* ncached, const int32_t* tables, int32_t max_blocks,
                      int32_t B, int32_t T, void* stream) {
     if (T == 0) return 0;
-    int grid = T < 148 * 16 ? T : 148 * 16;
     auto s = static_cast<cudaStream_t>(stream);
-#define CW_LAUNCH_APPEND(DD)                                                                                    \
-    append_kv_kernel<DD><<<grid, 128, 0, s>>>(                                                                  \
+    // threads per CTA: the multiple of 32 (<= 128) that leaves the fewest idle lanes in the last round over the token's
+    // units (8B: 384 units = 3 x 128; 70B: 640 = 5 x 128; Qwen2.5-7B: 288 = 3 x 96) — idle lanes are bytes not in flight
+    const int units = (cfg.num_q_heads + 2 * cfg.num_kv_heads) * (cfg.head_dim / 16);
+    int threads = 128, best_waste = 1 << 30;
+    for (int t = 128; t >= 64; t -= 32) {
+        const int waste = (units + t - 1) / t * t - units;
+        if (waste < best_waste) { best_waste = waste; threads = t; }
+    }
+    const int per_sm = 2048 / threads;
+    int grid = T < 148 * per_sm ? T : 148 * per_sm;
+#define CW_LAUNCH_APPEND(DD, TT)                                                                                \
+    append_kv_kernel<DD, TT><<<grid, TT, 0, s>>>(                                                               \
         (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, (__nv_bfloat16*)q_roped,     \
         (__nv_bfloat16*)cfg.k_pool, (__nv_bfloat16*)cfg.v_pool, (const float*)cfg.rope_table, cu, ncached,      \
         tables, max_blocks, B, T, cfg.num_q_heads, cfg.num_kv_heads, cfg.max_position)
-    if (cfg.head_dim == 128) CW_LAUNCH_APPEND(128); else CW_LAUNCH_APPEND(64);
+#define CW_LAUNCH_APPEND_D(DD)                                                                                  \
+    do {                                                                                                        \
+        if (threads == 128) CW_LAUNCH_APPEND(DD, 128);                                                          \
+        else if (threads == 96) CW_LAUNCH_APPEND(DD, 96);                                                       \
+        else CW_LAUNCH_APPEND(DD, 64);                                                                          \
+    } while (0)
+    if (cfg.head_dim == 128) CW_LAUNCH_APPEND_D(128); else CW_LAUNCH_APPEND_D(64);
+#undef CW_LAUNCH_APPEND_D
 #undef CW_LAUNCH_APPEND
     return (int)cudaGetLastError();
 }
