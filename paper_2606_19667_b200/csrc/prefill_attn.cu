@@ -462,6 +462,7 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
             const int ntok = wg ? w.ntok1 : w.ntok0;
             if (ntok == 0) continue;
             const int limit = w.pos0 + tl;                 // last visible key (inclusive); rows past the tile end are never stored
+            const bool row_valid = row < ntok * g;         // rows past the tile end hold stale Q: they must not steer the warp
             const int n_tiles = tiles_for(w.pos0 + wg * tpt + ntok);
 
             float m_ref = -INFINITY, l_sum = 0.f;
@@ -538,7 +539,7 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                             sv[i >> 1][(i & 1) * 16 + (e >> 1)] = ptx::pack_bf16x2(p.x, p.y);   // packed P: 64 registers
                         }
                     const float psum = ((ps[0].x + ps[0].y) + (ps[1].x + ps[1].y)) + ((ps[2].x + ps[2].y) + (ps[3].x + ps[3].y));
-                    if (spec && __any_sync(0xffffffffu, !(psum <= kSpecLimit))) {
+                    if (spec && __any_sync(0xffffffffu, row_valid && !(psum <= kSpecLimit))) {
                         spec = false;
                         continue;
                     }
