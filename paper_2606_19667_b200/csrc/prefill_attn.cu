@@ -73,10 +73,6 @@ __device__ __forceinline__ Item load_item(const int4* __restrict__ work, int idx
     const int4 a = ld_item_half(work + 2 * idx), b = ld_item_half(work + 2 * idx + 1);
     return Item{a.x, a.y, a.z, a.w, b.x, b.y, b.z};
 }
-__device__ __forceinline__ Item load_item_head(const int4* __restrict__ work, int idx) {   // pos0, ntok0, ntok1, tok0 only
-    const int4 a = ld_item_half(work + 2 * idx);
-    return Item{a.x, a.y, a.z, a.w, 0, 0, 0};
-}
 
 // exp2 on the FMA pipe for a share of the scores (the MUFU unit, 16 exp2 / clk / SM, is the softmax bottleneck):
 // 2^x = 2^round(x) * 2^f, f = x - round(x) in [-0.5, 0.5]; 2^f by a degree-3 polynomial (max rel. error 7.8e-5, P is
