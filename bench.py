@@ -177,7 +177,7 @@ class Workload:
         if st["event"] is not None:
             st["event"].synchronize()
         hi = lo + (expect.B if self.sequential else self.Bmax + 1)
-        a = self.ctx.cw_admit_batch(self.doc_ids[lo:hi], self.strategy == "greedy", self.trace.doc_tokens,
+        a = self.ctx.cw_admit_batch(self.doc_ids[lo:hi], self.strategy, self.trace.doc_tokens,
                                     self.queries[lo:hi], self.max_blocks, out=st["np"])
         if a["admitted"] != expect.B:
             raise RuntimeError(f"admission diverged: {a['admitted']} != {expect.B}")
@@ -470,6 +470,46 @@ def run_sweep(args):
     return cells
 
 
+def run_arms(args):
+    """Ordering arms of the paper's Table 4 on the bench configuration: retrieval, sorted, recency,
+    greedy (Algorithm 1), exhaustive.  One JSON line per arm with hit blocks, suffix tokens, attention flops, host admission
+    time and prefill ms, then a summary line with the share of the exhaustive arm's gain that greedy reaches."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback")
+    device = "cuda:0"
+    res = {}
+    for arm in ("retrieval", "sorted", "recency", "greedy", "exhaustive"):
+        wl = Workload(args.config, arm, device, want_e2e=False, device_inputs=True)
+        for _ in range(max(3, args.warmup)):
+            wl.step()
+        ev = []
+        ms_total = timed(torch, lambda: wl.step(ev), args.steps, None) / args.steps
+        app = sum(e[0].elapsed_time(e[1]) for e in ev) / args.steps
+        att = sum(e[1].elapsed_time(e[2]) for e in ev) / args.steps
+        t0 = time.perf_counter()
+        for _ in range(3):                                   # host admission alone (a1-a6 for all requests)
+            wl.ctx.cw_reset()
+            lo = 0
+            for w in wl.waves:
+                st, a = wl._admit(lo, w)
+                wl.ctx.cw_release_batch(a["reqs"][:w.B])
+                lo += w.B
+        host_ms = (time.perf_counter() - t0) / 3 * 1e3
+        res[arm] = {"arm": arm, "hit_blocks": wl.hit_blocks, "suffix_tokens": wl.T, "attn_flops": wl.flops,
+                    "prefill_ms": app + att, "append_ms": app, "attn_ms": att, "step_ms": ms_total,
+                    "host_admission_ms": host_ms, "host_us_per_request": 1e3 * host_ms / wl.cfg.n_req}
+        print(json.dumps(res[arm]), flush=True)
+        del wl
+        torch.cuda.empty_cache()
+    r, g, x = res["retrieval"], res["greedy"], res["exhaustive"]
+    share = lambda key: (r[key] - g[key]) / (r[key] - x[key]) if r[key] != x[key] else None
+    print(json.dumps({"summary": "greedy's share of the exhaustive arm's reduction vs retrieval order",
+                      "in_attn_flops": share("attn_flops"), "in_prefill_ms": share("prefill_ms"),
+                      "in_suffix_tokens": share("suffix_tokens"), "paper": "97.5 % of the oracle's TTFT reduction (PAPER.md:208)"}),
+          flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -481,12 +521,15 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--skip-retrieval", action="store_true")
     ap.add_argument("--device-inputs", action="store_true", help="timing-only: draw q,k,v on the device (no e2e leg)")
+    ap.add_argument("--arms", action="store_true", help="ordering arms of the paper's Table 4 on --config, one JSON line per arm")
     ap.add_argument("--sweep", action="store_true", help="overlap x top-k sweep (BASELINE.json configs[2]), one JSON line per cell")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.oracle_requests is None:
         args.oracle_requests = {1: 4, 2: 16 if args.impl == "ours" else 4, 4: 1, 5: 1}[args.config]
-    if args.sweep:
+    if args.arms:
+        run_arms(args)
+    elif args.sweep:
         run_sweep(args)
     elif args.impl == "reference":
         run_reference(args)

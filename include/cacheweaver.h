@@ -98,6 +98,20 @@ int cw_predict(cw_ctx* ctx, const int64_t* order, int32_t k, int32_t* out_prefix
  * path, stamp last_seq on every node of it; nodes outside the recency window are pruned lazily. */
 int cw_observe(cw_ctx* ctx, const int64_t* ordered_doc_ids, int32_t k);
 
+/* Ordering arms the paper compares with (Table 4; readings in DESIGN.md §2):
+ *   CW_ARM_RETRIEVAL  the retrieval order as given
+ *   CW_ARM_GREEDY     Algorithm 1 (cw_order)
+ *   CW_ARM_SORTED     ascending document id ("lexicographic sorting", a canonical query-independent order)
+ *   CW_ARM_RECENCY    documents served most recently first (index of the last cw_observe call containing the document,
+ *                     descending; never-served documents last; ties keep retrieval rank)
+ *   CW_ARM_EXHAUSTIVE of all k! orders (k <= 8) the one whose prompt matches the most resident blocks (peek lookups on
+ *                     the real block index); first maximiser in lexicographic order of retrieval-rank indices.  Needs the
+ *                     tokens: doc_tokens [num_docs, doc_len], query_tokens [q_len] (HOST; may be NULL for the other arms).
+ * out_order[k] (host); *out_pred_prefix_docs = l(O,T) of the chosen order (may be NULL).  Pure: no state change. */
+enum { CW_ARM_RETRIEVAL = 0, CW_ARM_GREEDY = 1, CW_ARM_SORTED = 2, CW_ARM_RECENCY = 3, CW_ARM_EXHAUSTIVE = 4 };
+int cw_order_arm(cw_ctx* ctx, int32_t arm, const int64_t* doc_ids, int32_t k, const int32_t* doc_tokens, int32_t num_docs,
+                 int32_t doc_len, const int32_t* query_tokens, int32_t q_len, int64_t* out_order, int32_t* out_pred_prefix_docs);
+
 /* ---- prefix cache, host (PAPER.md:33 chained block hashes; PAPER.md:129 block eviction) -------------- */
 /* chain[i] = FNV1a64(LE64(chain[i-1]) || 16 x LE32(token)), chain[-1] = hash_salt, i < floor(n/16). */
 int cw_hash_chain(cw_ctx* ctx, const int32_t* tokens, int32_t n, uint64_t* out_chain);
@@ -115,7 +129,7 @@ int cw_release(cw_ctx* ctx, int64_t req);
 int cw_reset(cw_ctx* ctx);
 /* Admission of a wave in ONE call: steps a1..a6 (+a2) for requests r = 0..B-1, in order (DESIGN.md reading
  * "requests of a batch are admitted sequentially on the host"):
- *     O_r = reorder ? Algorithm1(doc_ids[r]) : doc_ids[r];                      (cw_order / cw_predict)
+ *     O_r = cw_order_arm(arm = reorder, doc_ids[r])      (0 = retrieval order, 1 = Algorithm 1, 2.. = the other arms)
  *     tokens = doc_tokens[O_r[0]] || ... || doc_tokens[O_r[k-1]] || query_tokens[r];   (prompt assembly)
  *     (req, table, n_cached) = cw_lookup(tokens);  cw_observe(O_r)
  * All pointers HOST.  doc_ids [B,k] in retrieval rank; doc_tokens [num_docs, doc_len]; query_tokens [B, q_len];

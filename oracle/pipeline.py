@@ -20,6 +20,7 @@ import tracegen
 from .attention import PagedPool, attention_suffix, attention_full
 from .blocks import BlockManager, NoSpace, chain_hashes
 from .ordering import KnowledgeTree
+from .strategies import RecencyOrder, order_exhaustive, order_sorted
 
 
 @dataclass
@@ -47,11 +48,13 @@ def attention_flops(Hq, D, n, c):
 
 
 def run_trace(trace, strategy: str = "greedy", compute: bool = True, requests=None, sample_rows=None):
-    """strategy: 'greedy' (Algorithm 1) | 'retrieval' (identity, the comparison arm PAPER.md:155).
+    """strategy: 'greedy' (Algorithm 1) | 'retrieval' (identity, the comparison arm PAPER.md:155) | 'sorted' | 'recency' |
+    'exhaustive' (the arms of Table 4, oracle/strategies.py).
     compute=False does the host path only (order / lookup / tables).
     """
     cfg = trace.cfg
     tree = KnowledgeTree(cfg.H)
+    recency = RecencyOrder()
     bm = BlockManager(cfg.NB, eager_register=True)
     pool = PagedPool(cfg.NB, cfg.Hkv, cfg.D) if compute else None
     res = RunResult()
@@ -81,6 +84,15 @@ def run_trace(trace, strategy: str = "greedy", compute: bool = True, requests=No
             O, depth = tree.order(D)
         elif strategy == "retrieval":
             O, depth = list(D), tree.ell(D)
+        elif strategy == "sorted":
+            O = order_sorted(D)
+            depth = tree.ell(O)
+        elif strategy == "recency":
+            O = recency.order(D)
+            depth = tree.ell(O)
+        elif strategy == "exhaustive":
+            O, _ = order_exhaustive(list(D), lambda o: 16 * bm.match(tracegen.assemble_prompt(trace, r, o)))
+            depth = tree.ell(O)
         else:
             raise ValueError(strategy)
         tokens = tracegen.assemble_prompt(trace, r, O)
@@ -92,6 +104,7 @@ def run_trace(trace, strategy: str = "greedy", compute: bool = True, requests=No
             close_wave()
             continue                        # retry the same request in the next wave (order() is pure)
         tree.observe(O)
+        recency.observe(O)
         rr = RequestResult(r, O, depth, tokens, table, c, wave)
         res.requests.append(rr)
         wave_open.append((rr, req_id))

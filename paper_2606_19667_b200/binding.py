@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_PKG, "libcacheweaver.so")
 
 CW_OK, CW_ERR_INVALID, CW_ERR_NO_SPACE, CW_ERR_BAD_HANDLE, CW_ERR_CUDA = 0, -1, -2, -3, -4
 BLOCK_SIZE = 16
+ARMS = {"retrieval": 0, "greedy": 1, "sorted": 2, "recency": 3, "exhaustive": 4}     # CW_ARM_* (cacheweaver.h)
 
 
 class CwConfig(C.Structure):
@@ -66,6 +67,7 @@ def load_library(build_if_missing: bool = True):
         "cw_q_roped_offset": (i64, [p(CwConfig), i32, i32, i32, i32]),
         "cw_order": (C.c_int, [vp, p(i64), i32, p(i64), p(i32)]),
         "cw_predict": (C.c_int, [vp, p(i64), i32, p(i32)]),
+        "cw_order_arm": (C.c_int, [vp, i32, p(i64), i32, p(i32), i32, i32, p(i32), i32, p(i64), p(i32)]),
         "cw_observe": (C.c_int, [vp, p(i64), i32]),
         "cw_hash_chain": (C.c_int, [vp, p(i32), i32, p(C.c_uint64)]),
         "cw_lookup": (C.c_int, [vp, p(i32), i32, i32, p(i64), p(i32), p(i32)]),
@@ -90,7 +92,7 @@ def load_library(build_if_missing: bool = True):
 
 
 EXPORTS = ["cw_create", "cw_destroy", "cw_strerror", "cw_last_error", "cw_stats", "cw_pool_bytes", "cw_pool_offset", "cw_q_roped_offset",
-           "cw_order", "cw_predict", "cw_observe", "cw_hash_chain", "cw_lookup", "cw_release", "cw_free_list",
+           "cw_order", "cw_predict", "cw_order_arm", "cw_observe", "cw_hash_chain", "cw_lookup", "cw_release", "cw_free_list",
            "cw_reset", "cw_admit_batch", "cw_release_batch",
            "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_gather_kv", "cw_prefill_host_ws_bytes",
            "cw_prefill_host"]
@@ -167,6 +169,20 @@ class Context:
         self._check(self.lib.cw_order(self.h, _i64p(d), len(d), _i64p(out), C.byref(depth)))
         return out.tolist(), depth.value
 
+    def cw_order_arm(self, arm, doc_ids, doc_tokens=None, query_tokens=None):
+        """arm: ARMS name or id.  doc_tokens int32 [num_docs, doc_len], query_tokens int32 [q_len] (exhaustive arm only)."""
+        arm = ARMS[arm] if isinstance(arm, str) else int(arm)
+        d = np.ascontiguousarray(doc_ids, dtype=np.int64)
+        out = np.empty_like(d)
+        depth = C.c_int32()
+        dt = _np_i32(doc_tokens) if doc_tokens is not None else None
+        qt = _np_i32(query_tokens) if query_tokens is not None else None
+        self._check(self.lib.cw_order_arm(self.h, arm, _i64p(d), len(d), _i32p(dt) if dt is not None else None,
+                                          dt.shape[0] if dt is not None else 0, dt.shape[1] if dt is not None else 0,
+                                          _i32p(qt) if qt is not None else None, len(qt) if qt is not None else 0,
+                                          _i64p(out), C.byref(depth)))
+        return out.tolist(), depth.value
+
     def cw_predict(self, order):
         d = np.ascontiguousarray(order, dtype=np.int64)
         depth = C.c_int32()
@@ -220,7 +236,7 @@ class Context:
         nc = o.get("n_cached", np.empty(B, dtype=np.int32))
         cu = o.get("cu", np.empty(B + 1, dtype=np.int32))
         adm = C.c_int32()
-        self._check(self.lib.cw_admit_batch(self.h, _i64p(doc_ids), B, k, int(bool(reorder)), _i32p(doc_tokens), num_docs,
+        self._check(self.lib.cw_admit_batch(self.h, _i64p(doc_ids), B, k, ARMS[reorder] if isinstance(reorder, str) else int(reorder), _i32p(doc_tokens), num_docs,
                                             doc_len, _i32p(query_tokens), q_len, _i64p(orders), _i32p(pred), _i64p(reqs),
                                             _i32p(tables), max_blocks, _i32p(nc), _i32p(cu), C.byref(adm)))
         return dict(orders=orders, pred=pred, reqs=reqs, tables=tables, n_cached=nc, cu=cu, admitted=adm.value)

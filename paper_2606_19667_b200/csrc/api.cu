@@ -158,6 +158,55 @@ int cw_observe(cw_ctx* ctx, const int64_t* ordered, int32_t k) {
     if (!ctx || k < 0 || (k > 0 && !ordered)) return fail(ctx, CW_ERR_INVALID, "cw_observe: bad argument");
     if (has_duplicates(ordered, k)) return fail(ctx, CW_ERR_INVALID, "cw_observe: duplicate document id");
     ctx->tree->observe(ordered, k);
+    for (int i = 0; i < k; ++i) ctx->last_served[ordered[i]] = ctx->tree->seq();
+    return CW_OK;
+}
+
+int cw_order_arm(cw_ctx* ctx, int32_t arm, const int64_t* doc_ids, int32_t k, const int32_t* doc_tokens, int32_t num_docs,
+                 int32_t doc_len, const int32_t* query_tokens, int32_t q_len, int64_t* out_order, int32_t* out_pred) {
+    if (!ctx || k < 0 || (k > 0 && (!doc_ids || !out_order)) || arm < CW_ARM_RETRIEVAL || arm > CW_ARM_EXHAUSTIVE)
+        return fail(ctx, CW_ERR_INVALID, "cw_order_arm: bad argument");
+    if (has_duplicates(doc_ids, k)) return fail(ctx, CW_ERR_INVALID, "cw_order_arm: duplicate document id");
+    if (arm == CW_ARM_GREEDY) {
+        ctx->tree->order(doc_ids, k, out_order);
+    } else if (arm == CW_ARM_RETRIEVAL) {
+        std::memcpy(out_order, doc_ids, sizeof(int64_t) * (size_t)k);
+    } else if (arm == CW_ARM_SORTED) {
+        std::memcpy(out_order, doc_ids, sizeof(int64_t) * (size_t)k);
+        std::sort(out_order, out_order + k);
+    } else if (arm == CW_ARM_RECENCY) {
+        std::memcpy(out_order, doc_ids, sizeof(int64_t) * (size_t)k);
+        auto served = [&](int64_t d) {
+            auto it = ctx->last_served.find(d);
+            return it == ctx->last_served.end() ? (int64_t)0 : it->second;
+        };
+        std::stable_sort(out_order, out_order + k, [&](int64_t a, int64_t b) { return served(a) > served(b); });
+    } else {
+        if (k > 8 || doc_len < 0 || q_len < 0 || (k > 0 && !doc_tokens) || (q_len > 0 && !query_tokens))
+            return fail(ctx, CW_ERR_INVALID, "cw_order_arm: exhaustive search needs k <= 8 and the tokens");
+        for (int i = 0; i < k; ++i)
+            if (doc_ids[i] < 0 || doc_ids[i] >= num_docs) return fail(ctx, CW_ERR_INVALID, "cw_order_arm: doc id out of range");
+        const int32_t n = k * doc_len + q_len;
+        if (n <= 0) return fail(ctx, CW_ERR_INVALID, "cw_order_arm: empty prompt");
+        std::vector<int32_t> tokens((size_t)n);
+        if (q_len) std::memcpy(tokens.data() + (size_t)k * doc_len, query_tokens, sizeof(int32_t) * (size_t)q_len);
+        std::vector<int> perm((size_t)k);
+        for (int i = 0; i < k; ++i) perm[(size_t)i] = i;
+        std::vector<uint64_t> chain;
+        int32_t best = -1;
+        do {   // permutations in lexicographic order of retrieval-rank indices; keep the first maximiser
+            for (int i = 0; i < k; ++i)
+                std::memcpy(tokens.data() + (size_t)i * doc_len, doc_tokens + (size_t)doc_ids[perm[(size_t)i]] * doc_len,
+                            sizeof(int32_t) * (size_t)doc_len);
+            ctx->blocks->chain(tokens.data(), n, chain);
+            const int32_t m = ctx->blocks->match(chain, n);
+            if (m > best) {
+                best = m;
+                for (int i = 0; i < k; ++i) out_order[i] = doc_ids[perm[(size_t)i]];
+            }
+        } while (std::next_permutation(perm.begin(), perm.end()));
+    }
+    if (out_pred) *out_pred = ctx->tree->predict(out_order, k);
     return CW_OK;
 }
 
@@ -195,6 +244,7 @@ int cw_reset(cw_ctx* ctx) {
     delete ctx->blocks;
     ctx->tree = new cw::KnowledgeTree(ctx->cfg.recency_window);
     ctx->blocks = new cw::BlockManager(ctx->cfg.num_blocks, ctx->cfg.eager_register != 0, ctx->cfg.hash_salt);
+    ctx->last_served.clear();
     ctx->last_error.clear();
     return CW_OK;
 }
@@ -222,11 +272,10 @@ int cw_admit_batch(cw_ctx* ctx, const int64_t* doc_ids, int32_t B, int32_t k, in
         for (int i = 0; i < k; ++i)
             if (D[i] < 0 || D[i] >= num_docs) return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: doc id out of range");
         if (has_duplicates(D, k)) return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: duplicate document id");
-        if (reorder) {
-            out_pred[r] = ctx->tree->order(D, k, O);
-        } else {
-            std::memcpy(O, D, sizeof(int64_t) * (size_t)k);
-            out_pred[r] = ctx->tree->predict(O, k);
+        {
+            const int rc = cw_order_arm(ctx, reorder, D, k, doc_tokens, num_docs, doc_len,
+                                        q_len ? query_tokens + (size_t)r * q_len : nullptr, q_len, O, out_pred + r);
+            if (rc != CW_OK) return rc;
         }
         for (int i = 0; i < k; ++i)
             std::memcpy(tokens.data() + (size_t)i * doc_len, doc_tokens + (size_t)O[i] * doc_len, sizeof(int32_t) * (size_t)doc_len);
@@ -237,6 +286,7 @@ int cw_admit_batch(cw_ctx* ctx, const int64_t* doc_ids, int32_t B, int32_t k, in
         if (rc != CW_OK) return rc;
         for (int32_t i = nblk; i < max_blocks; ++i) table[i] = 0;
         ctx->tree->observe(O, k);
+        for (int i = 0; i < k; ++i) ctx->last_served[O[i]] = ctx->tree->seq();
         out_cu[r + 1] = out_cu[r] + (n - out_nc[r]);
         *out_admitted = r + 1;
     }

@@ -98,6 +98,8 @@ struct cw_ctx {
     std::string last_error;
     bool host_only;
     int num_sms;
+    // comparison arms (cw_order_arm): index of the last cw_observe call whose order contained the document
+    std::unordered_map<int64_t, int64_t> last_served;
     // cw_prefill_host pipeline: copy streams and per-chunk events (created on first use, destroyed with the context)
     void* copy_in_stream = nullptr;
     void* copy_out_stream = nullptr;

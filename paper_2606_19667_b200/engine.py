@@ -79,8 +79,8 @@ class TraceRunner:
             O, depth = self.ctx.cw_order(D)
         elif self.strategy == "retrieval":
             O, depth = list(D), self.ctx.cw_predict(D)
-        else:
-            raise ValueError(self.strategy)
+        else:                                              # sorted | recency | exhaustive (cw_order_arm)
+            O, depth = self.ctx.cw_order_arm(self.strategy, D, self.trace.doc_tokens, self.trace.query_tokens[r])
         tokens = tracegen.assemble_prompt(self.trace, r, O)
         req, table, c = self.ctx.cw_lookup(tokens)        # raises NoSpace with state unchanged
         self.ctx.cw_observe(O)
@@ -177,7 +177,7 @@ def admit_waves(ctx: Context, trace: tracegen.Trace, strategy: str = "greedy", r
     step = None if (force_waves or cfg.admission == "waves") else 1
     while i < len(todo):
         j = len(todo) if step is None else min(len(todo), i + step)
-        a = ctx.cw_admit_batch(doc_ids[i:j], strategy == "greedy", trace.doc_tokens, queries[i:j], cfg.blocks_per_req)
+        a = ctx.cw_admit_batch(doc_ids[i:j], strategy, trace.doc_tokens, queries[i:j], cfg.blocks_per_req)
         m = a["admitted"]
         if m == 0:
             raise NoSpace(-2, "a single request does not fit the pool")
