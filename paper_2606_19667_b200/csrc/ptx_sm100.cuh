@@ -3,6 +3,7 @@
 // Bit layouts follow the PTX ISA "tcgen05 matrix descriptor" / "instruction descriptor" tables.
 #pragma once
 #include <cstdint>
+#include <cstdio>
 
 namespace cw { namespace ptx {
 
@@ -39,7 +40,17 @@ __device__ __forceinline__ bool mbar_test_wait(uint32_t bar, uint32_t parity) {
     return ok != 0;
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+#ifdef CW_WATCHDOG   // debug builds only: a wait that lasts > ~1 s reports its barrier and traps instead of hanging the GPU
+    const long long t0 = clock64();
+    while (!mbar_try_wait(bar, parity)) {
+        if (clock64() - t0 > 2000000000ll) {
+            printf("cw watchdog: block %d thread %d stuck on mbarrier smem+%u parity %u\n", blockIdx.x, threadIdx.x, bar, parity);
+            __trap();
+        }
+    }
+#else
     while (!mbar_try_wait(bar, parity)) {}
+#endif
 }
 
 // ---- proxies / fences -------------------------------------------------------------------------------------
@@ -98,6 +109,53 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64
         "setp.ne.b32 p, %4, 0;\n\t"
         "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
         :: "r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// S[tmem, 128 x N] = Q K^T over the whole head dim in ONE asm statement: D/16 MMAs (K = 16 each) whose descriptors are
+// derived inside the block, so the compiler cannot hoist D/16 descriptor pairs into vector registers.  Operand tiles are
+// the 128B-swizzled K-major layouts of this library: k-step ks reads 32 bytes further inside a 64-dim half, the second
+// half of Q sits 128 rows x 128 B (= 1024 descriptor units) further, the second half of a K chunk 1024 B (= 64 units).
+template <int D>
+__device__ __forceinline__ void umma_ss_qk(uint32_t d_tmem, uint64_t q_desc, uint64_t k_desc, uint32_t idesc) {
+    static_assert(D == 64 || D == 128, "head dim");
+    if constexpr (D == 128) {
+        asm volatile(
+            "{\n\t.reg .pred p0, p1;\n\t.reg .b64 a, b;\n\t"
+            "setp.ne.b32 p0, 0, 0;\n\tsetp.eq.b32 p1, 0, 0;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p0;\n\t"
+            "add.s64 a, %1, 2;\n\tadd.s64 b, %2, 2;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p1;\n\t"
+            "add.s64 a, %1, 4;\n\tadd.s64 b, %2, 4;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p1;\n\t"
+            "add.s64 a, %1, 6;\n\tadd.s64 b, %2, 6;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p1;\n\t"
+            "add.s64 a, %1, 1024;\n\tadd.s64 b, %2, 64;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p1;\n\t"
+            "add.s64 a, %1, 1026;\n\tadd.s64 b, %2, 66;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p1;\n\t"
+            "add.s64 a, %1, 1028;\n\tadd.s64 b, %2, 68;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p1;\n\t"
+            "add.s64 a, %1, 1030;\n\tadd.s64 b, %2, 70;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p1;\n\t}"
+            :: "r"(d_tmem), "l"(q_desc), "l"(k_desc), "r"(idesc) : "memory");
+    } else {
+        asm volatile(
+            "{\n\t.reg .pred p0, p1;\n\t.reg .b64 a, b;\n\t"
+            "setp.ne.b32 p0, 0, 0;\n\tsetp.eq.b32 p1, 0, 0;\n\t"
+            "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p0;\n\t"
+            "add.s64 a, %1, 2;\n\tadd.s64 b, %2, 2;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p1;\n\t"
+            "add.s64 a, %1, 4;\n\tadd.s64 b, %2, 4;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p1;\n\t"
+            "add.s64 a, %1, 6;\n\tadd.s64 b, %2, 6;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], a, b, %3, p1;\n\t}"
+            :: "r"(d_tmem), "l"(q_desc), "l"(k_desc), "r"(idesc) : "memory");
+    }
+}
+// O[tmem, 128 x D] (+)= P V for a full 64-key chunk in ONE asm statement: 4 MMAs (16 keys each).  P (bf16) is read from
+// TMEM, 8 columns per k-step; V is the MN-major operand, 16 keys = `v_step` descriptor units further per k-step.
+// accumulate == 0 only for the first chunk of an item (the first k-step then overwrites O).
+template <int D>
+__device__ __forceinline__ void umma_ts_pv4(uint32_t d_tmem, uint32_t p_tmem, uint64_t v_desc, uint32_t idesc, uint32_t accumulate) {
+    constexpr int kStep = (2 * (D / 64) * 1024) >> 4;      // 16 keys = two 8-key groups
+    asm volatile(
+        "{\n\t.reg .pred p0, p1;\n\t.reg .b64 b;\n\t.reg .b32 t;\n\t"
+        "setp.ne.b32 p0, %4, 0;\n\tsetp.eq.b32 p1, 0, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p0;\n\t"
+        "add.s32 t, %1, 8;\n\tadd.s64 b, %2, %5;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], [t], b, %3, p1;\n\t"
+        "add.s32 t, %1, 16;\n\tadd.s64 b, %2, %6;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], [t], b, %3, p1;\n\t"
+        "add.s32 t, %1, 24;\n\tadd.s64 b, %2, %7;\n\ttcgen05.mma.cta_group::1.kind::f16 [%0], [t], b, %3, p1;\n\t}"
+        :: "r"(d_tmem), "r"(p_tmem), "l"(v_desc), "r"(idesc), "r"(accumulate), "n"(kStep), "n"(2 * kStep), "n"(3 * kStep)
+        : "memory");
 }
 // all previously issued MMAs of this thread complete -> one arrival on the mbarrier (implies fence::before_thread_sync)
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
