@@ -284,6 +284,7 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
         // the loader.  The whole warp runs the control flow (operands stay in uniform registers); one elected lane issues.
         auto mma_role = [&](auto wtag) {
             constexpr int W = decltype(wtag)::value;
+            if (!ptx::elect_one()) return;          // ONE thread runs the whole role: every operand is trivially uniform
             constexpr uint32_t kIdescQK = ptx::umma_idesc_bf16(kTileM, 0, 0, 0);      // N is added per chunk
             constexpr uint32_t kIdescPV = ptx::umma_idesc_bf16(kTileM, D, 0, 1);
             constexpr uint32_t kGroupStride = (D / 64) * 1024;        // bytes between 8-key groups of a K/V chunk
@@ -307,7 +308,14 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
             uint32_t kslot = 0, kph = 0;             // ring slot (even) and phase of the K chunk at the QK^T cursor
             uint32_t vslot = 1, vph = 0;             // ring slot (odd) and phase of the V chunk at the PV cursor
             uint32_t qf = 0, oi = 0, n_item = 0;
-            Geo gc = geo_of(get_item(0, false)), gn = gc;
+            auto fetch = [&](uint32_t n) {              // single-thread version of get_item
+                const uint32_t slot = n % kSchedSlots;
+                ptx::mbar_wait(bar(BAR_SCHED_FULL + slot), (n / kSchedSlots) & 1u);
+                const int4 a = *reinterpret_cast<const int4*>(smem + L::kSched + slot * 32);
+                ptx::mbar_arrive(bar(BAR_SCHED_EMPTY + slot));
+                return Item{a.x, a.y, a.z, a.w, 0, 0, 0};
+            };
+            Geo gc = geo_of(fetch(0)), gn = gc;
             bool q_on_next = false;                  // QK^T cursor: chunk qj of the current / the next item
             int qj = 0;
             // pass the chunk at the QK^T cursor: S_w[sc & 1] = Q_w K^T if the tile reads it; false at the end of what is known
@@ -327,15 +335,12 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                     ptx::tc_fence_after();
                     const uint32_t b = sc & 1u;
                     const uint32_t idesc = kIdescQK | ((uint32_t)(blocks_in_chunk(nkv_x, qj) * 2) << 17);   // N = 16 * blocks
-                    if (ptx::elect_one()) {
-                        ptx::umma_ss_qk<D>(tS + b * 64u, qdesc, kdesc0 + (uint64_t)((kslot * L::kKVBytes) >> 4), idesc);
-                        ptx::umma_commit(bar(BAR_S_FULL + W * 2 + (int)b));
-                        ptx::umma_commit(bar(BAR_RING + NS + kslot));
-                        if (qj + 1 == n_x) ptx::umma_commit(bar(BAR_Q_EMPTY + W));      // last read of Q_w: hand the buffer back
-                    }
-                    __syncwarp();
+                    ptx::umma_ss_qk<D>(tS + b * 64u, qdesc, kdesc0 + (uint64_t)((kslot * L::kKVBytes) >> 4), idesc);
+                    ptx::umma_commit(bar(BAR_S_FULL + W * 2 + (int)b));
+                    ptx::umma_commit(bar(BAR_RING + NS + kslot));
+                    if (qj + 1 == n_x) ptx::umma_commit(bar(BAR_Q_EMPTY + W));          // last read of Q_w: hand the buffer back
                     ++sc;
-                } else if (lane == 0) {
+                } else {
                     ptx::mbar_arrive(bar(BAR_RING + NS + kslot));
                 }
                 kslot += 2;
@@ -348,7 +353,7 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 return true;
             };
             while (gc.nt > 0) {
-                gn = geo_of(get_item(n_item + 1, false));
+                gn = geo_of(fetch(n_item + 1));
                 while (gq - gp < 2u && qk_step()) {}
                 for (int j = 0; j < gc.nt; ++j) {
                     // ---- O_w (+)= P_w[pc & 1] V(j) ----
@@ -362,21 +367,18 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                         }
                         ptx::tc_fence_after();
                         const int ksteps = blocks_in_chunk(gc.nkv, j);            // 16-key steps that hold a visible key
-                        if (ptx::elect_one()) {
-                            const uint64_t vd = vdesc0 + (uint64_t)((vslot * L::kKVBytes) >> 4);
-                            if (ksteps == kChunk / 16) {
-                                ptx::umma_ts_pv4<D>(tO, tS + b * 64u, vd, kIdescPV, j > 0 ? 1u : 0u);
-                            } else {
-                                for (int ks = 0; ks < ksteps; ++ks)
-                                    ptx::umma_ts(tO, tS + b * 64u + (uint32_t)ks * 8u, vd + (uint64_t)((ks * 2 * kGroupStride) >> 4),
-                                                 kIdescPV, (j > 0 || ks > 0) ? 1u : 0u);
-                            }
-                            ptx::umma_commit(bar(BAR_RING + NS + vslot));          // V slot free; also "PV done" for the lazy rescale
-                            if (j + 1 == gc.n) ptx::umma_commit(bar(BAR_O_FULL + W));   // O_w complete: the epilogue may read it
+                        const uint64_t vd = vdesc0 + (uint64_t)((vslot * L::kKVBytes) >> 4);
+                        if (ksteps == kChunk / 16) {
+                            ptx::umma_ts_pv4<D>(tO, tS + b * 64u, vd, kIdescPV, j > 0 ? 1u : 0u);
+                        } else {
+                            for (int ks = 0; ks < ksteps; ++ks)
+                                ptx::umma_ts(tO, tS + b * 64u + (uint32_t)ks * 8u, vd + (uint64_t)((ks * 2 * kGroupStride) >> 4),
+                                             kIdescPV, (j > 0 || ks > 0) ? 1u : 0u);
                         }
-                        __syncwarp();
+                        ptx::umma_commit(bar(BAR_RING + NS + vslot));              // V slot free; also "PV done" for the lazy rescale
+                        if (j + 1 == gc.n) ptx::umma_commit(bar(BAR_O_FULL + W));       // O_w complete: the epilogue may read it
                         ++pc;
-                    } else if (lane == 0) {
+                    } else {
                         ptx::mbar_arrive(bar(BAR_RING + NS + vslot));
                     }
                     vslot += 2;
@@ -394,9 +396,9 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 gc = gn;
                 ++n_item;
             }
-            __syncwarp();
         };
         if (warp == 12) mma_role(std::integral_constant<int, 0>{}); else mma_role(std::integral_constant<int, 1>{});
+        __syncwarp();
       }
     } else if (warp >= 8) {
         // ================================ epilogue (warps 8-11): O_w / l_w -> bf16 -> global ================================
