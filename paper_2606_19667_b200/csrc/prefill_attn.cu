@@ -87,7 +87,7 @@ __device__ __forceinline__ Item load_item(const int4* __restrict__ work, int idx
 // 7.8e-5, P is rounded to bf16 = 3.9e-3 afterwards); round(x) through the 1.5*2^23 magic constant, spliced into the
 // exponent field.  x is clamped to [-125, 126]: the low side flushes to ~0, the high side (only reachable on the
 // speculative path, where x is taken against a stale maximum) saturates at 2^126 so that the row sum trips kSpecLimit.
-constexpr int kPolyPeriod = 4;   // of every kPolyPeriod score pairs ...
+constexpr int kPolyPeriod = 8;   // of every kPolyPeriod score pairs ...
 constexpr int kPolyCount = 1;    // ... this many use the polynomial
 __device__ __forceinline__ float2 exp2_poly2(float2 x) {
     const float kMagic = 12582912.f;
