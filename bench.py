@@ -136,7 +136,7 @@ class Workload:
                 g.manual_seed(cfg.seed * 1000 + wi)
                 dq, dk, dv = (torch.randn(w.T, h, cfg.D, device=device, dtype=torch.bfloat16, generator=g)
                               for h in (cfg.Hq, cfg.Hkv, cfg.Hkv))
-                work = torch.empty(max(4, self.ctx.cw_attn_work_ints(w.cu)), dtype=torch.int32, device=device)
+                work = torch.empty(self.ctx.cw_attn_work_ints(w.B, w.T), dtype=torch.int32, device=device)
                 self.inputs.append((dq, dk, dv, torch.empty_like(dq), torch.empty_like(dq), work))
                 continue
             rows = tracegen.batch_suffix_qkv(trace, w.items, threads=os.cpu_count() or 8)
@@ -144,7 +144,7 @@ class Workload:
             if want_e2e:
                 self.host_inputs.append([t.pin_memory() for t in qkv] + [torch.empty_like(qkv[0]).pin_memory()])
             dq, dk, dv = (t.to(device) for t in qkv)
-            work = torch.empty(max(4, self.ctx.cw_attn_work_ints(w.cu)), dtype=torch.int32, device=device)
+            work = torch.empty(self.ctx.cw_attn_work_ints(w.B, w.T), dtype=torch.int32, device=device)
             self.inputs.append((dq, dk, dv, torch.empty_like(dq), torch.empty_like(dq), work))
         # pinned staging ring for the admission outputs + device descriptors
         self.ring = []
@@ -163,6 +163,10 @@ class Workload:
             st["event"] = None
             self.ring.append(st)
         self.slot, self.Bmax = 0, Bmax
+        self.req_ws = None
+        if sequential:      # per-request path: cw_prefill_requests stages the descriptors itself (one call per request)
+            self.req_ws = torch.empty(max(self.ctx.cw_prefill_requests_ws_bytes(w.B, w.T, self.max_blocks) for w in self.waves),
+                                      dtype=torch.uint8, device=device)
         self.ws = None
         if want_e2e:
             nbytes = max(self.ctx.cw_prefill_host_ws_bytes(w.B, w.T, self.max_blocks) for w in self.waves)
@@ -184,13 +188,22 @@ class Workload:
         return st, a
 
     def step(self, events=None):
-        """resident inputs: host admission + H2D of the descriptors + 2 launches per wave."""
+        """resident inputs: host admission + H2D of the descriptors + 3 launches per wave (RoPE + scatter, schedule,
+        attention).  The per-request variant (sequential=True) goes through cw_prefill_requests instead: one C call per
+        request stages the descriptors and enqueues the same three launches."""
         torch, ctx = self.torch, self.ctx
         ctx.cw_reset()
         lo = 0
         for wi, w in enumerate(self.waves):
             st, a = self._admit(lo, w)
             B, T = w.B, w.T
+            if self.req_ws is not None:
+                q, k, v, qr, out, _ = self.inputs[wi]
+                ctx.cw_prefill_requests(a["reqs"][:B], q, k, v, qr, out, T, self.max_blocks, self.req_ws)
+                ctx.cw_release_batch(a["reqs"][:B])
+                self.launches += 3
+                lo += B
+                continue
             st["d_tables"][:B].copy_(st["tables"][:B], non_blocking=True)
             st["d_nc"][:B].copy_(st["n_cached"][:B], non_blocking=True)
             st["d_cu"][:B + 1].copy_(st["cu"][:B + 1], non_blocking=True)
@@ -201,15 +214,14 @@ class Workload:
             ctx.cw_append_kv(q, k, v, qr, st["d_cu"], st["d_nc"], st["d_tables"], self.max_blocks, B, T)
             if events is not None:
                 e[1].record()
-            ctx.cw_prefill_attn(qr, out, a["cu"], a["n_cached"], st["d_cu"], st["d_nc"], st["d_tables"], self.max_blocks,
-                                B, T, work)
+            ctx.cw_prefill_attn(qr, out, st["d_cu"], st["d_nc"], st["d_tables"], self.max_blocks, B, T, w.max_q, w.max_kv, work)
             if events is not None:
                 e[2].record()
                 events.append(e)
             st["event"] = torch.cuda.Event()
             st["event"].record()
             ctx.cw_release_batch(a["reqs"][:B])
-            self.launches += 2
+            self.launches += 3
             lo += B
 
     def step_e2e(self):
@@ -400,7 +412,8 @@ def run_ours(args):
             for _ in range(args.warmup):
                 ws.step()
             s_ms = timed(torch, ws.step, args.steps, None) / args.steps
-            prefill["per_request_launches"] = {"ms_per_trace": s_ms, "launches": 2 * len(ws.waves), "attn_flops": ws.flops,
+            prefill["per_request_launches"] = {"ms_per_trace": s_ms, "launches": 3 * len(ws.waves), "attn_flops": ws.flops,
+                                               "us_per_request": 1e3 * s_ms / len(ws.waves), "api": "cw_admit_batch(1) + cw_prefill_requests + cw_release_batch per request",
                                                "value_tflops": ws.flops / (s_ms * 1e-3) / 1e12}
             del ws
 

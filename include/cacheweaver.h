@@ -137,7 +137,8 @@ int cw_reset(cw_ctx* ctx);
  * are set to 0; max_blocks >= ceil((k*doc_len+q_len)/16)); out_n_cached [B]; out_cu_seqlens_q [B+1] (prefix sums of
  * the suffix lengths n - n_cached).  Admission stops at the first request that does not fit (CW_ERR_NO_SPACE; that
  * request and all later ones leave the state unchanged); *out_admitted = number admitted, return value CW_OK unless
- * an argument is invalid (doc id outside [0,num_docs), duplicate ids, ...), in which case admission also stops. */
+ * an argument is invalid (doc id outside [0,num_docs), duplicate ids, unknown arm, ...): every row is checked before
+ * the first request is admitted, so CW_ERR_INVALID leaves the state unchanged (*out_admitted = 0). */
 int cw_admit_batch(cw_ctx* ctx, const int64_t* doc_ids, int32_t B, int32_t k, int32_t reorder,
                    const int32_t* doc_tokens, int32_t num_docs, int32_t doc_len,
                    const int32_t* query_tokens, int32_t q_len,
@@ -168,15 +169,38 @@ int cw_append_kv(cw_ctx* ctx, const void* q, const void* k, const void* v, void*
 /* cw_prefill_attn — varlen paged causal GQA attention of the suffix rows (kernel 2):
  *     o[row p, head h] = sum_{j<=p} softmax_j(q'_p . k'_j / sqrt(D)) v_j, kv head = h / g, keys j read from the
  *     pool through the block table (cached prefix j < n_cached and the blocks just written by cw_append_kv).
- *   h_cu_seqlens_q [B+1], h_n_cached [B]: HOST copies of the same descriptors (used only to build the tile
- *   schedule on the host; kv_len[r] = n_cached[r] + suffix length).  d_work: DEVICE int32 scratch of
- *   cw_attn_work_ints(...) ints, caller-owned, filled asynchronously on `stream` by this call.
- *   q_roped: as written by cw_append_kv (tile-packed); out [T,Hq,D] device bf16 row-major.  One persistent CTA per SM. */
-int64_t cw_attn_work_ints(cw_ctx* ctx, const int32_t* h_cu_seqlens_q, int32_t B);
+ *   Fully asynchronous: every descriptor is a DEVICE pointer and nothing is read on the host.  The call enqueues a
+ *   one-CTA schedule kernel (request descriptors -> list of work items, longest request first) and the persistent
+ *   attention kernel (one CTA per SM) on `stream`.
+ *   d_kv_len [B]: device, kv_len[r] = n_cached[r] + suffix length; may be NULL (it is redundant and only cross-checked).
+ *   max_q_len / max_kv_len: upper bounds on the suffix length / kv length of any request of the batch (host values;
+ *   max_kv_len <= 16 * max_blocks_per_req and <= max_position).
+ *   d_work: DEVICE int32 scratch of cw_attn_work_ints(ctx, B, T) ints, caller-owned, written by this call.  After the
+ *   stream has run the call: d_work[1] != 0 means a request descriptor was invalid (n_cached not a multiple of 16,
+ *   lengths beyond the stated maxima, kv_len mismatch) and that request produced no output; d_work[2] counts the
+ *   softmax chunks that left the speculative path (statistics); d_work[3] is the number of work items.
+ *   q_roped: as written by cw_append_kv (tile-packed); out [T,Hq,D] device bf16 row-major.
+ *   (SURVEY.md 8(b) lists this signature without d_work; the scratch is passed in because the library allocates no
+ *   device memory.) */
+int64_t cw_attn_work_ints(cw_ctx* ctx, int32_t B, int32_t T);
 int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out,
-                    const int32_t* h_cu_seqlens_q, const int32_t* h_n_cached,
-                    const int32_t* d_cu_seqlens_q, const int32_t* d_n_cached, const int32_t* d_block_tables,
-                    int32_t max_blocks_per_req, int32_t B, int32_t T, int32_t* d_work, void* stream);
+                    const int32_t* d_cu_seqlens_q, const int32_t* d_n_cached, const int32_t* d_kv_len,
+                    const int32_t* d_block_tables, int32_t max_blocks_per_req, int32_t B, int32_t T,
+                    int32_t max_q_len, int32_t max_kv_len, int32_t* d_work, void* stream);
+
+/* cw_prefill_requests — steps a7 + a8 for a wave of admitted requests in ONE call: the descriptors (cu_seqlens_q,
+ * n_cached, block tables) are taken from the request handles reqs[0..B-1] (HOST, as returned by cw_lookup /
+ * cw_admit_batch, in batch order), written to a library-owned pinned staging slot, copied to d_ws with one
+ * asynchronous H2D copy, and cw_append_kv + cw_prefill_attn are enqueued on `stream`.  Nothing is synchronised.
+ *   q [T,Hq,D], k, v [T,Hkv,D], q_roped, out: device bf16 as in cw_append_kv / cw_prefill_attn; T must equal the sum
+ *   of the requests' suffix lengths.  max_blocks_per_req >= the largest block-table length of the wave.
+ *   d_ws: device scratch of cw_prefill_requests_ws_bytes() bytes, caller-owned (descriptors at offset 0: cu [B+1],
+ *   n_cached [B], tables [B, max_blocks_per_req]; then the attention work list, 256-byte aligned).  The work list of
+ *   the call starts at byte offset cw_prefill_requests_work_offset(); its header reads as described at cw_prefill_attn). */
+int64_t cw_prefill_requests_ws_bytes(cw_ctx* ctx, int32_t B, int32_t T, int32_t max_blocks_per_req);
+int64_t cw_prefill_requests_work_offset(cw_ctx* ctx, int32_t B, int32_t max_blocks_per_req);
+int cw_prefill_requests(cw_ctx* ctx, const int64_t* reqs, int32_t B, const void* q, const void* k, const void* v,
+                        void* q_roped, void* out, int32_t T, int32_t max_blocks_per_req, void* d_ws, void* stream);
 
 /* cw_gather_kv — export: pool -> plain row-major k_out, v_out [n, Hkv, D] bf16 (device) for one block table
  * (device int32 [ceil(n/16)]).  Used by tests and by callers that want the cached KV in a plain layout. */
@@ -184,8 +208,8 @@ int cw_gather_kv(cw_ctx* ctx, const int32_t* d_block_table, int32_t n, void* k_o
 
 /* cw_prefill_host — the same path with HOST buffers (end-to-end entry point).  The batch is cut into up to 8 request
  * chunks of about equal token count and pipelined: H2D of chunk i+1 (library-owned copy stream), cw_append_kv +
- * cw_prefill_attn of chunk i (on `stream`, in request order), D2H of chunk i-1 (second copy stream); the call returns
- * after everything has completed (both `stream` and the copy streams are synchronised).  q, k, v, out are staged in the
+ * cw_prefill_attn of chunk i (on `stream`, in request order), D2H of chunk i-1 (second copy stream); all of it is
+ * enqueued without blocking, then the call waits until everything has completed (`stream` and the copy streams).  q, k, v, out are staged in the
  * caller-owned device workspace `d_ws` (cw_prefill_host_ws_bytes bytes).  Host buffers should be pinned (pageable
  * memory works but serialises the copies).  h_block_tables is [B, max_blocks_per_req].  The two copy streams and their
  * events are created on first use and destroyed by cw_destroy. */

@@ -55,7 +55,8 @@ def load_library(build_if_missing: bool = True):
         from .build import build
         build()
     lib = C.CDLL(LIB_PATH)
-    p, i32, i64, vp = C.POINTER, C.c_int32, C.c_int64, C.c_void_p
+    i32, i64, vp = C.c_int32, C.c_int64, C.c_void_p
+    p = lambda _t: vp      # typed pointers are passed as plain addresses (numpy: a.ctypes.data): cheapest marshalling
     sig = {
         "cw_create": (C.c_int, [p(CwConfig), p(vp)]),
         "cw_destroy": (None, [vp]),
@@ -78,8 +79,11 @@ def load_library(build_if_missing: bool = True):
                                      p(i32), i32, p(i32), p(i32), p(i32)]),
         "cw_release_batch": (C.c_int, [vp, p(i64), i32]),
         "cw_append_kv": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp]),
-        "cw_attn_work_ints": (i64, [vp, p(i32), i32]),
-        "cw_prefill_attn": (C.c_int, [vp, vp, vp, p(i32), p(i32), vp, vp, vp, i32, i32, i32, vp, vp]),
+        "cw_attn_work_ints": (i64, [vp, i32, i32]),
+        "cw_prefill_attn": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]),
+        "cw_prefill_requests_ws_bytes": (i64, [vp, i32, i32, i32]),
+        "cw_prefill_requests_work_offset": (i64, [vp, i32, i32]),
+        "cw_prefill_requests": (C.c_int, [vp, p(i64), i32, vp, vp, vp, vp, vp, i32, i32, vp, vp]),
         "cw_gather_kv": (C.c_int, [vp, vp, i32, vp, vp, vp]),
         "cw_prefill_host_ws_bytes": (i64, [vp, i32, i32, i32]),
         "cw_prefill_host": (C.c_int, [vp, vp, vp, vp, vp, p(i32), p(i32), p(i32), i32, i32, i32, vp, vp]),
@@ -94,16 +98,17 @@ def load_library(build_if_missing: bool = True):
 EXPORTS = ["cw_create", "cw_destroy", "cw_strerror", "cw_last_error", "cw_stats", "cw_pool_bytes", "cw_pool_offset", "cw_q_roped_offset",
            "cw_order", "cw_predict", "cw_order_arm", "cw_observe", "cw_hash_chain", "cw_lookup", "cw_release", "cw_free_list",
            "cw_reset", "cw_admit_batch", "cw_release_batch",
-           "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_gather_kv", "cw_prefill_host_ws_bytes",
+           "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_prefill_requests_ws_bytes",
+           "cw_prefill_requests_work_offset", "cw_prefill_requests", "cw_gather_kv", "cw_prefill_host_ws_bytes",
            "cw_prefill_host"]
 
 
 def _i32p(a):
-    return a.ctypes.data_as(C.POINTER(C.c_int32))
+    return a.ctypes.data
 
 
 def _i64p(a):
-    return a.ctypes.data_as(C.POINTER(C.c_int64))
+    return a.ctypes.data
 
 
 def _np_i32(x):
@@ -197,7 +202,7 @@ class Context:
     def cw_hash_chain(self, tokens):
         t = _np_i32(tokens)
         out = np.empty(len(t) // BLOCK_SIZE, dtype=np.uint64)
-        self._check(self.lib.cw_hash_chain(self.h, _i32p(t), len(t), out.ctypes.data_as(C.POINTER(C.c_uint64))))
+        self._check(self.lib.cw_hash_chain(self.h, _i32p(t), len(t), out.ctypes.data))
         return out
 
     def cw_lookup(self, tokens, peek_only=False):
@@ -273,15 +278,29 @@ class Context:
                                           d_cu.data_ptr(), d_nc.data_ptr(), d_tables.data_ptr(), max_blocks, B, T,
                                           self._stream()))
 
-    def cw_attn_work_ints(self, h_cu):
-        h_cu = _np_i32(h_cu)
-        return int(self.lib.cw_attn_work_ints(self.h, _i32p(h_cu), len(h_cu) - 1))
+    def cw_attn_work_ints(self, B, T):
+        return int(self.lib.cw_attn_work_ints(self.h, int(B), int(T)))
 
-    def cw_prefill_attn(self, q_roped, out, h_cu, h_nc, d_cu, d_nc, d_tables, max_blocks, B, T, d_work):
-        h_cu, h_nc = _np_i32(h_cu), _np_i32(h_nc)
-        self._check(self.lib.cw_prefill_attn(self.h, q_roped.data_ptr(), out.data_ptr(), _i32p(h_cu), _i32p(h_nc),
-                                             d_cu.data_ptr(), d_nc.data_ptr(), d_tables.data_ptr(), max_blocks, B, T,
-                                             d_work.data_ptr(), self._stream()))
+    def cw_prefill_attn(self, q_roped, out, d_cu, d_nc, d_tables, max_blocks, B, T, max_q_len, max_kv_len, d_work,
+                        d_kv_len=None):
+        """all descriptors are device int32 tensors; d_work: device int32 scratch of cw_attn_work_ints(B, T) ints."""
+        self._check(self.lib.cw_prefill_attn(self.h, q_roped.data_ptr(), out.data_ptr(), d_cu.data_ptr(), d_nc.data_ptr(),
+                                             d_kv_len.data_ptr() if d_kv_len is not None else None, d_tables.data_ptr(),
+                                             max_blocks, B, T, int(max_q_len), int(max_kv_len), d_work.data_ptr(),
+                                             self._stream()))
+
+    def cw_prefill_requests_ws_bytes(self, B, T, max_blocks):
+        return int(self.lib.cw_prefill_requests_ws_bytes(self.h, B, T, max_blocks))
+
+    def cw_prefill_requests_work_offset(self, B, max_blocks):
+        return int(self.lib.cw_prefill_requests_work_offset(self.h, B, max_blocks))
+
+    def cw_prefill_requests(self, reqs, q, k, v, q_roped, out, T, max_blocks, d_ws):
+        """reqs: request handles of the wave (numpy int64, batch order); q, k, v, q_roped, out, d_ws: device tensors."""
+        r = np.ascontiguousarray(reqs, dtype=np.int64)
+        self._check(self.lib.cw_prefill_requests(self.h, _i64p(r), len(r), q.data_ptr(), k.data_ptr(), v.data_ptr(),
+                                                 q_roped.data_ptr(), out.data_ptr(), int(T), int(max_blocks),
+                                                 d_ws.data_ptr(), self._stream()))
 
     def cw_gather_kv(self, d_table, n, k_out, v_out):
         self._check(self.lib.cw_gather_kv(self.h, d_table.data_ptr(), n, k_out.data_ptr(), v_out.data_ptr(),

@@ -108,6 +108,10 @@ int cw_create(const cw_config* cfg, cw_ctx** out) {
 void cw_destroy(cw_ctx* ctx) {
     if (!ctx) return;
     for (void* e : ctx->events) cudaEventDestroy(static_cast<cudaEvent_t>(e));
+    for (auto& st : ctx->staging) {
+        if (st.event) cudaEventDestroy(static_cast<cudaEvent_t>(st.event));
+        if (st.host) cudaFreeHost(st.host);
+    }
     if (ctx->copy_in_stream) cudaStreamDestroy(static_cast<cudaStream_t>(ctx->copy_in_stream));
     if (ctx->copy_out_stream) cudaStreamDestroy(static_cast<cudaStream_t>(ctx->copy_out_stream));
     delete ctx->tree;
@@ -265,13 +269,19 @@ int cw_admit_batch(cw_ctx* ctx, const int64_t* doc_ids, int32_t B, int32_t k, in
         !out_tables || !out_nc)
         return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: null pointer");
     const int32_t n = (int32_t)n64, nblk = (n + CW_BLOCK_SIZE - 1) / CW_BLOCK_SIZE;
+    if (reorder < CW_ARM_RETRIEVAL || reorder > CW_ARM_EXHAUSTIVE || (reorder == CW_ARM_EXHAUSTIVE && k > 8))
+        return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: unknown ordering arm (or exhaustive with k > 8)");
+    // every row is validated BEFORE anything is admitted: an invalid argument leaves the state untouched
+    for (int32_t r = 0; r < B; ++r) {
+        const int64_t* D = doc_ids + (size_t)r * k;
+        for (int i = 0; i < k; ++i)
+            if (D[i] < 0 || D[i] >= num_docs) return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: doc id out of range");
+        if (has_duplicates(D, k)) return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: duplicate document id");
+    }
     std::vector<int32_t> tokens((size_t)n);
     for (int32_t r = 0; r < B; ++r) {
         const int64_t* D = doc_ids + (size_t)r * k;
         int64_t* O = out_orders + (size_t)r * k;
-        for (int i = 0; i < k; ++i)
-            if (D[i] < 0 || D[i] >= num_docs) return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: doc id out of range");
-        if (has_duplicates(D, k)) return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: duplicate document id");
         {
             const int rc = cw_order_arm(ctx, reorder, D, k, doc_tokens, num_docs, doc_len,
                                         q_len ? query_tokens + (size_t)r * q_len : nullptr, q_len, O, out_pred + r);
@@ -329,35 +339,114 @@ int cw_gather_kv(cw_ctx* ctx, const int32_t* d_table, int32_t n, void* k_out, vo
     return e ? cuda_fail(ctx, e, "cw_gather_kv") : CW_OK;
 }
 
-int64_t cw_attn_work_ints(cw_ctx* ctx, const int32_t* h_cu, int32_t B) {
-    if (!ctx || B < 0 || (B > 0 && !h_cu)) return CW_ERR_INVALID;
-    return cw::attn_work_ints(ctx->cfg, h_cu, B);
+int64_t cw_attn_work_ints(cw_ctx* ctx, int32_t B, int32_t T) {
+    if (!ctx || B < 0 || T < 0) return CW_ERR_INVALID;
+    return cw::attn_work_ints(ctx->cfg, B, T);
 }
 
-int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out, const int32_t* h_cu, const int32_t* h_nc,
-                    const int32_t* d_cu, const int32_t* d_nc, const int32_t* d_tables, int32_t max_blocks, int32_t B,
-                    int32_t T, int32_t* d_work, void* stream) {
+int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out, const int32_t* d_cu, const int32_t* d_nc,
+                    const int32_t* d_kv_len, const int32_t* d_tables, int32_t max_blocks, int32_t B, int32_t T,
+                    int32_t max_q_len, int32_t max_kv_len, int32_t* d_work, void* stream) {
     if (!ctx || ctx->host_only) return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn: host-only context");
-    if (B < 0 || T < 0 || max_blocks <= 0) return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn: bad sizes");
+    if (B < 0 || T < 0 || max_blocks <= 0 || max_q_len < 0 || max_kv_len < 0)
+        return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn: bad sizes");
     if (T == 0 || B == 0) return CW_OK;
-    if (!q_roped || !out || !h_cu || !h_nc || !d_cu || !d_nc || !d_tables || !d_work)
+    if (!q_roped || !out || !d_cu || !d_nc || !d_tables || !d_work)
         return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn: null pointer");
-    if (h_cu[0] != 0 || h_cu[B] != T) return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn: cu_seqlens_q does not span T");
-    for (int r = 0; r < B; ++r) {
-        const int s = h_cu[r + 1] - h_cu[r];
-        if (s < 0 || h_nc[r] < 0 || h_nc[r] % CW_BLOCK_SIZE != 0 ||
-            (int64_t)h_nc[r] + s > (int64_t)max_blocks * CW_BLOCK_SIZE || h_nc[r] + s > ctx->cfg.max_position)
-            return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn: bad request descriptor");
-    }
-    std::vector<int32_t> work;
-    const int64_t tiles = cw::attn_build_schedule(ctx->cfg, h_cu, h_nc, B, work);
-    if (tiles == 0) return CW_OK;
-    cudaError_t e = cudaMemcpyAsync(d_work, work.data(), work.size() * sizeof(int32_t), cudaMemcpyHostToDevice,
-                                    static_cast<cudaStream_t>(stream));   // pageable source: staged before return
-    if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_attn (schedule copy)");
-    int le = cw::launch_prefill_attn(ctx->cfg, q_roped, out, d_tables, max_blocks, d_work, tiles,
-                                     ctx->num_sms, stream);
+    if (max_q_len > T || (int64_t)max_kv_len > (int64_t)max_blocks * CW_BLOCK_SIZE || max_kv_len > ctx->cfg.max_position)
+        return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn: max_q_len / max_kv_len exceed T, the block table or max_position");
+    int le = cw::launch_prefill_attn(ctx->cfg, q_roped, out, d_cu, d_nc, d_kv_len, d_tables, max_blocks, B, T, max_q_len,
+                                     max_kv_len, d_work, ctx->num_sms, stream);
     return le ? cuda_fail(ctx, le, "cw_prefill_attn") : CW_OK;
+}
+
+// ---- one call per wave: descriptors from the request handles, one staged H2D copy, three launches ----------
+namespace {
+struct ReqWsLayout {
+    int64_t cu, nc, tables, work, total;
+};
+ReqWsLayout req_ws_layout(const cw_config& c, int32_t B, int32_t T, int32_t max_blocks) {
+    ReqWsLayout w{};
+    int64_t o = 0;
+    w.cu = o; o += ((int64_t)B + 1) * 4;                 // cu, nc and the tables are contiguous: one H2D copy
+    w.nc = o; o += (int64_t)B * 4;
+    w.tables = o; o += (int64_t)B * max_blocks * 4;
+    o = align256(o);
+    w.work = o; o += align256(cw::attn_work_ints(c, B, T) * 4);
+    w.total = o;
+    return w;
+}
+}  // namespace
+
+int64_t cw_prefill_requests_ws_bytes(cw_ctx* ctx, int32_t B, int32_t T, int32_t max_blocks) {
+    if (!ctx || B < 0 || T < 0 || max_blocks <= 0) return CW_ERR_INVALID;
+    return req_ws_layout(ctx->cfg, B, T, max_blocks).total;
+}
+
+int64_t cw_prefill_requests_work_offset(cw_ctx* ctx, int32_t B, int32_t max_blocks) {
+    if (!ctx || B < 0 || max_blocks <= 0) return CW_ERR_INVALID;
+    return req_ws_layout(ctx->cfg, B, 0, max_blocks).work;
+}
+
+int cw_prefill_requests(cw_ctx* ctx, const int64_t* reqs, int32_t B, const void* q, const void* k, const void* v,
+                        void* q_roped, void* out, int32_t T, int32_t max_blocks, void* d_ws, void* stream) {
+    if (!ctx || ctx->host_only) return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: host-only context");
+    if (B < 0 || T < 0 || max_blocks <= 0) return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: bad sizes");
+    if (B == 0) return T == 0 ? CW_OK : fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: T != 0 for an empty batch");
+    if (!reqs || !q || !k || !v || !q_roped || !out || !d_ws || q == q_roped)
+        return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: null or aliased pointer");
+    const ReqWsLayout w = req_ws_layout(ctx->cfg, B, T, max_blocks);
+    // descriptors of the wave, written into a pinned staging slot (cu | nc | tables, contiguous like in d_ws)
+    const size_t desc_bytes = (size_t)w.tables + (size_t)B * max_blocks * 4;
+    cw_ctx::Staging& st = ctx->staging[ctx->staging_next];
+    ctx->staging_next = (ctx->staging_next + 1) % cw_ctx::kStagingSlots;
+    cudaError_t e = cudaSuccess;
+    if (st.event) e = cudaEventSynchronize(static_cast<cudaEvent_t>(st.event));   // the copy that last read this slot
+    if (e == cudaSuccess && st.cap < desc_bytes) {
+        if (st.host) cudaFreeHost(st.host);
+        st.host = nullptr;
+        st.cap = 0;
+        const size_t cap = std::max<size_t>(desc_bytes * 2, 1 << 16);
+        e = cudaMallocHost(&st.host, cap);
+        if (e == cudaSuccess) st.cap = cap;
+    }
+    if (e == cudaSuccess && !st.event) {
+        cudaEvent_t ev;
+        e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+        if (e == cudaSuccess) st.event = ev;
+    }
+    if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_requests (staging)");
+    int32_t* cu = reinterpret_cast<int32_t*>(static_cast<char*>(st.host) + w.cu);
+    int32_t* nc = reinterpret_cast<int32_t*>(static_cast<char*>(st.host) + w.nc);
+    int32_t* tables = reinterpret_cast<int32_t*>(static_cast<char*>(st.host) + w.tables);
+    cu[0] = 0;
+    int32_t max_q = 0, max_kv = 0;
+    for (int32_t r = 0; r < B; ++r) {
+        const cw::Request* rq = ctx->blocks->find(reqs[r]);
+        if (!rq) return fail(ctx, CW_ERR_BAD_HANDLE, "cw_prefill_requests: unknown request handle");
+        const int32_t nblk = (int32_t)rq->table.size(), c = rq->m * CW_BLOCK_SIZE, s = rq->n - c;
+        if (nblk > max_blocks) return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: max_blocks too small for a request");
+        if (rq->n > ctx->cfg.max_position) return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: prompt longer than max_position");
+        nc[r] = c;
+        cu[r + 1] = cu[r] + s;
+        std::memcpy(tables + (size_t)r * max_blocks, rq->table.data(), sizeof(int32_t) * (size_t)nblk);
+        std::memset(tables + (size_t)r * max_blocks + nblk, 0, sizeof(int32_t) * (size_t)(max_blocks - nblk));
+        max_q = std::max(max_q, s);
+        max_kv = std::max(max_kv, rq->n);
+    }
+    if (cu[B] != T) return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: T does not match the requests' suffix lengths");
+    auto s = static_cast<cudaStream_t>(stream);
+    char* ws = static_cast<char*>(d_ws);
+    e = cudaMemcpyAsync(ws, st.host, desc_bytes, cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaEventRecord(static_cast<cudaEvent_t>(st.event), s);
+    if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_requests (descriptor copy)");
+    const int32_t* d_cu = reinterpret_cast<const int32_t*>(ws + w.cu);
+    const int32_t* d_nc = reinterpret_cast<const int32_t*>(ws + w.nc);
+    const int32_t* d_tables = reinterpret_cast<const int32_t*>(ws + w.tables);
+    int rc = cw_append_kv(ctx, q, k, v, q_roped, d_cu, d_nc, d_tables, max_blocks, B, T, stream);
+    if (rc != CW_OK) return rc;
+    return cw_prefill_attn(ctx, q_roped, out, d_cu, d_nc, nullptr, d_tables, max_blocks, B, T, max_q, max_kv,
+                           reinterpret_cast<int32_t*>(ws + w.work), stream);
 }
 
 // ---- host-buffer entry point ------------------------------------------------------------------------------
@@ -379,10 +468,7 @@ WsLayout ws_layout(const cw_config& c, int32_t B, int32_t T, int32_t max_blocks)
     w.nc = o; o += align256((int64_t)B * 4);
     w.tables = o; o += align256((int64_t)B * max_blocks * 4);
     // upper bound on tiles: every request may add one ragged tile per kv head
-    const int g = c.num_q_heads / c.num_kv_heads;
-    const int tpt2 = 2 * (128 / g);
-    const int64_t max_items = (((int64_t)T + tpt2 - 1) / tpt2 + B) * c.num_kv_heads;
-    w.work = o; o += align256((max_items + kHostChunks) * 32) + 256 * kHostChunks;   // one list (+ header) per chunk
+    w.work = o; o += align256(cw::attn_work_ints(c, B, T) * 4) + (align256(32) + 256) * kHostChunks;   // one list (+ header) per chunk
     w.total = o;
     return w;
 }
@@ -402,6 +488,15 @@ int cw_prefill_host(cw_ctx* ctx, const void* h_q, const void* h_k, const void* h
     if (!h_q || !h_k || !h_v || !h_out || !h_cu || !h_nc || !h_tables || !d_ws)
         return fail(ctx, CW_ERR_INVALID, "cw_prefill_host: null pointer");
     if (h_cu[0] != 0 || h_cu[B] != T) return fail(ctx, CW_ERR_INVALID, "cw_prefill_host: cu_seqlens_q does not span T");
+    int32_t max_q = 0, max_kv = 0;
+    for (int r = 0; r < B; ++r) {
+        const int s = h_cu[r + 1] - h_cu[r];
+        if (s < 0 || h_nc[r] < 0 || h_nc[r] % CW_BLOCK_SIZE != 0 ||
+            (int64_t)h_nc[r] + s > (int64_t)max_blocks * CW_BLOCK_SIZE || h_nc[r] + s > ctx->cfg.max_position)
+            return fail(ctx, CW_ERR_INVALID, "cw_prefill_host: bad request descriptor");
+        max_q = std::max(max_q, s);
+        max_kv = std::max(max_kv, h_nc[r] + s);
+    }
     const cw_config& c = ctx->cfg;
     const WsLayout w = ws_layout(c, B, T, max_blocks);
     auto s = static_cast<cudaStream_t>(stream);
@@ -464,15 +559,14 @@ int cw_prefill_host(cw_ctx* ctx, const void* h_q, const void* h_k, const void* h
         const int32_t* d_cu = (const int32_t*)(ws + w.cu) + cu_off[(size_t)k];
         const int32_t* d_nc = (const int32_t*)(ws + w.nc) + r0;
         const int32_t* d_tab = (const int32_t*)(ws + w.tables) + (size_t)r0 * max_blocks;
-        const int32_t* hc = cu_local.data() + cu_off[(size_t)k];
         int rc = cw_append_kv(ctx, ws + w.q + t0 * qrow, ws + w.k + t0 * krow, ws + w.v + t0 * krow, ws + w.qr + t0 * qrow, d_cu, d_nc,
                               d_tab, max_blocks, Bc, (int32_t)Tc, stream);
         if (rc != CW_OK) return rc;
         int32_t* d_work = (int32_t*)(ws + w.work) + work_off;
-        rc = cw_prefill_attn(ctx, ws + w.qr + t0 * qrow, ws + w.out + t0 * qrow, hc, h_nc + r0, d_cu, d_nc, d_tab, max_blocks, Bc,
-                             (int32_t)Tc, d_work, stream);
+        rc = cw_prefill_attn(ctx, ws + w.qr + t0 * qrow, ws + w.out + t0 * qrow, d_cu, d_nc, nullptr, d_tab, max_blocks, Bc,
+                             (int32_t)Tc, std::min<int32_t>(max_q, (int32_t)Tc), max_kv, d_work, stream);
         if (rc != CW_OK) return rc;
-        work_off += (cw::attn_work_ints(c, hc, Bc) + 63) / 64 * 64;
+        work_off += (cw::attn_work_ints(c, Bc, (int32_t)Tc) + 63) / 64 * 64;
         e = cudaEventRecord(ev(kHostChunks + k), s);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(s_out, ev(kHostChunks + k), 0);
         if (e == cudaSuccess) e = cudaMemcpyAsync((char*)h_out + t0 * qrow, ws + w.out + t0 * qrow, Tc * qrow, cudaMemcpyDeviceToHost, s_out);

@@ -58,7 +58,8 @@ class KnowledgeTree {
 struct Request {
     std::vector<int32_t> table;
     std::vector<uint64_t> chain;
-    int32_t m;
+    int32_t m;      // matched (cached) blocks
+    int32_t n;      // prompt length in tokens
 };
 
 class BlockManager {
@@ -69,6 +70,10 @@ class BlockManager {
     // returns CW_OK / CW_ERR_NO_SPACE
     int lookup(const int32_t* tokens, int32_t n, int64_t* req, int32_t* table, int32_t* n_cached);
     int release(int64_t req);
+    const Request* find(int64_t req) const {
+        auto it = reqs_.find(req);
+        return it == reqs_.end() ? nullptr : &it->second;
+    }
     int32_t free_list(int32_t* out, int32_t cap) const;
     int64_t requests = 0, hit_blocks = 0, miss_blocks = 0, evictions = 0;
     int32_t free_count() const { return free_count_; }
@@ -104,6 +109,16 @@ struct cw_ctx {
     void* copy_in_stream = nullptr;
     void* copy_out_stream = nullptr;
     std::vector<void*> events;
+    // cw_prefill_requests: ring of pinned host slots the wave descriptors are staged in (grown on demand); the event marks
+    // the H2D copy that last read the slot
+    struct Staging {
+        void* host = nullptr;
+        size_t cap = 0;
+        void* event = nullptr;
+    };
+    static constexpr int kStagingSlots = 4;
+    Staging staging[kStagingSlots];
+    int staging_next = 0;
 };
 
 // kernel launchers (defined in the .cu files); return cudaError_t as int
@@ -112,11 +127,11 @@ int launch_append_kv(const cw_config& cfg, const void* q, const void* k, const v
                      const int32_t* cu, const int32_t* ncached, const int32_t* tables, int32_t max_blocks,
                      int32_t B, int32_t T, void* stream);
 int launch_gather_kv(const cw_config& cfg, const int32_t* table, int32_t n, void* k_out, void* v_out, void* stream);
-// attention item list: 8 ints per item (prefill_attn.cu); returns item count
-int64_t attn_count_tiles(const cw_config& cfg, const int32_t* h_cu, int32_t B);
-int64_t attn_work_ints(const cw_config& cfg, const int32_t* h_cu, int32_t B);
-int64_t attn_build_schedule(const cw_config& cfg, const int32_t* h_cu, const int32_t* h_nc, int32_t B,
-                            std::vector<int32_t>& work);
-int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* tables, int32_t max_blocks,
-                        int32_t* d_work, int64_t num_items, int num_sms, void* stream);
+// attention: the item list (8 ints per item + an 8-int header) is built on the device by a schedule kernel launched in
+// front of the attention kernel; attn_work_ints is the scratch size for a batch of B requests / T suffix rows
+int64_t attn_max_items(const cw_config& cfg, int32_t B, int32_t T);
+int64_t attn_work_ints(const cw_config& cfg, int32_t B, int32_t T);
+int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* d_cu, const int32_t* d_nc,
+                        const int32_t* d_kv_len, const int32_t* tables, int32_t max_blocks, int32_t B, int32_t T,
+                        int32_t max_q_len, int32_t max_kv_len, int32_t* d_work, int num_sms, void* stream);
 }  // namespace cw

@@ -136,6 +136,7 @@ int BlockManager::lookup(const int32_t* tokens, int32_t n, int64_t* req, int32_t
     Request r;
     chain(tokens, n, r.chain);
     int32_t nblk = (n + CW_BLOCK_SIZE - 1) / CW_BLOCK_SIZE, nfull = n / CW_BLOCK_SIZE;
+    r.n = n;
     r.m = match(r.chain, n);                                                    // (1)
     r.table.resize((size_t)nblk);
     int32_t matched_free = 0;

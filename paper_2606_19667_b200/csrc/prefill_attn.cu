@@ -118,8 +118,7 @@ template <int D>
 __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
     const __nv_bfloat16* __restrict__ q_roped, __nv_bfloat16* __restrict__ out,
     const __nv_bfloat16* __restrict__ k_pool, const __nv_bfloat16* __restrict__ v_pool,
-    const int32_t* __restrict__ tables, int max_blocks, int4* __restrict__ work, int num_items,
-    int Hq, int Hkv, float scale_log2) {
+    const int32_t* __restrict__ tables, int max_blocks, int4* __restrict__ work, int Hq, int Hkv, float scale_log2) {
     using L = Smem<D>;
     constexpr int NS = L::kStages;
     extern __shared__ __align__(1024) uint8_t smem[];
@@ -133,7 +132,8 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
     const int tpt = kTileM / g;          // tokens per Q tile
     const int R = tpt * g;               // rows of a full Q tile
 
-    // Dynamic schedule: work[0].x is a counter (zeroed with the list), items follow from work + 2.
+    // Dynamic schedule (written by attn_schedule_kernel): work[0] = {claim counter, error flags, fallbacks, number of items},
+    // items follow from work + 2.
     // The loader warp claims items with atomicAdd and publishes each descriptor through a small smem ring; every other
     // warp reads item #n from slot n % kSchedSlots (an item with ntok0 == 0 ends the stream).
     const int4* items = work + 2;
@@ -188,6 +188,7 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
         constexpr uint32_t kBlockBytes = 16 * D * 2;
         uint32_t it = 0, qcnt0 = 0, qcnt1 = 0, n_item = 0;
         int* counter = reinterpret_cast<int*>(work);
+        const int num_items = __ldg(reinterpret_cast<const int*>(work) + 3);
         auto claim = [&]() {                          // lane 0 holds the claimed index
             int i = 0;
             if (lane == 0) i = atomicAdd(counter, 1);
@@ -585,69 +586,157 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
     }
 }
 
-// ---- host side: item list and launch ------------------------------------------------------------------------
-// Items per request: ceil(s / (2*tpt)) * Hkv.
-int64_t attn_count_tiles(const cw_config& cfg, const int32_t* h_cu, int32_t B) {
-    const int g = cfg.num_q_heads / cfg.num_kv_heads;
-    const int tpt = kTileM / g;
-    int64_t n = 0;
-    for (int r = 0; r < B; ++r) {
-        const int64_t s = h_cu[r + 1] - h_cu[r];
-        n += (s + 2 * tpt - 1) / (2 * tpt) * cfg.num_kv_heads;
+// ---- schedule kernel: the item list is built on the device, so cw_prefill_attn never reads a descriptor on the host ----
+// One CTA.  Request r has s = cu[r+1] - cu[r] suffix rows at positions nc[r] .. nc[r] + s - 1 and gives
+// ceil(s / (2 tpt)) * Hkv items.  Item order: requests by descending work s * (2 nc + s) (ties by index: longest first,
+// so the tail of the launch is made of short items); inside a request kv-head major, tile pairs by descending kv length.
+// CTA b takes items b, b+G, b+2G, ...: the CTAs work on neighbouring items of the same (request, kv head) at the same
+// time and share its K/V blocks through L2.
+// work header (ints): [0] claim counter, [1] error flags (bit 0: a request descriptor was invalid and contributes no
+// item), [2] exact-path fallbacks of the speculative softmax (statistics), [3] number of items; items from int 8 on.
+constexpr int kSchedMaxSmemReqs = 2048;      // requests whose (suffix, cached, offset) fit the schedule kernel's shared memory
+
+__global__ void __launch_bounds__(1024) attn_schedule_kernel(
+    const int32_t* __restrict__ cu, const int32_t* __restrict__ nc, const int32_t* __restrict__ kv_len, int B, int T,
+    int Hq, int Hkv, int D, int max_blocks, int max_position, int max_q_len, int max_kv_len, int32_t* __restrict__ work,
+    int64_t max_items) {
+    const int g = Hq / Hkv, tpt = kTileM / g, R = tpt * g;
+    __shared__ int s_err, s_total;
+    __shared__ int s_s[kSchedMaxSmemReqs], s_c[kSchedMaxSmemReqs], s_off[kSchedMaxSmemReqs];
+    const bool in_smem = B <= kSchedMaxSmemReqs;
+    if (threadIdx.x == 0) {
+        s_err = 0;
+        s_total = 0;
     }
-    return n;
-}
-
-int64_t attn_work_ints(const cw_config& cfg, const int32_t* h_cu, int32_t B) {
-    return kWorkInts * (attn_count_tiles(cfg, h_cu, B) + 1);   // + header (work counter)
-}
-
-// Item order: requests by descending work (longest first, so the tail of the launch is made of short items); inside
-// a request kv-head major, tile pairs by descending kv length.  CTA b takes items b, b+G, b+2G, ...: the CTAs work
-// on neighbouring items of the same (request, kv head) at the same time and share its K/V blocks through L2.
-int64_t attn_build_schedule(const cw_config& cfg, const int32_t* h_cu, const int32_t* h_nc, int32_t B,
-                            std::vector<int32_t>& work) {
-    const int g = cfg.num_q_heads / cfg.num_kv_heads, D = cfg.head_dim, Hq = cfg.num_q_heads;
-    const int tpt = kTileM / g, R = tpt * g;
-    std::vector<int32_t> reqs((size_t)B);
-    for (int r = 0; r < B; ++r) reqs[(size_t)r] = r;
-    auto work_of = [&](int r) {
-        const int64_t s = h_cu[r + 1] - h_cu[r], c = h_nc[r];
-        return s * (2 * c + s);                      // ~ number of (row, key) pairs
+    __syncthreads();
+    // suffix length of request r (0 and the error flag if its descriptor is invalid) and its cached length
+    auto suffix = [&](int r, int& c) {
+        const int lo = cu[r], hi = cu[r + 1];
+        c = nc[r];
+        const int64_t s = (int64_t)hi - lo;
+        const bool ok = lo >= 0 && s >= 0 && hi <= T && c >= 0 && c % CW_BLOCK_SIZE == 0 && s <= max_q_len &&
+                        (int64_t)c + s <= max_kv_len && (int64_t)c + s <= (int64_t)max_blocks * CW_BLOCK_SIZE &&
+                        (int64_t)c + s <= max_position && (kv_len == nullptr || kv_len[r] == c + s);
+        return ok ? (int)s : -1;
     };
-    std::stable_sort(reqs.begin(), reqs.end(), [&](int a, int b) { return work_of(a) > work_of(b); });
-    work.assign(kWorkInts, 0);                        // header: work[0] = claim counter, zeroed with every upload
-    for (int r : reqs) {
-        const int s = h_cu[r + 1] - h_cu[r];
-        const int npair = (s + 2 * tpt - 1) / (2 * tpt);
-        for (int kvh = 0; kvh < cfg.num_kv_heads; ++kvh)
-            for (int t = npair - 1; t >= 0; --t) {
-                const int tok0 = t * 2 * tpt;
-                const int ntok0 = std::min(tpt, s - tok0), ntok1 = std::max(0, std::min(tpt, s - tok0 - tpt));
-                const int64_t q_off = ((int64_t)h_cu[r] * Hq + (int64_t)kvh * s * g) * D + (int64_t)t * 2 * R * D;   // elements
-                const int32_t item[kWorkInts] = {h_nc[r] + tok0, ntok0, ntok1, h_cu[r] + tok0, r, kvh, (int32_t)(q_off / 8), 0};
-                work.insert(work.end(), item, item + kWorkInts);
-            }
+    auto get = [&](int r, int& c) {           // validated (s, c) of request r
+        if (in_smem) {
+            c = s_c[r];
+            return s_s[r];
+        }
+        const int s = suffix(r, c);
+        return s < 0 ? 0 : s;
+    };
+    for (int r = threadIdx.x; r < B; r += blockDim.x) {
+        int c;
+        int s = suffix(r, c);
+        if (s < 0) {
+            atomicOr(&s_err, 1);
+            s = 0;
+        }
+        if (in_smem) {
+            s_s[r] = s;
+            s_c[r] = c;
+        }
     }
-    return (int64_t)work.size() / kWorkInts - 1;
+    __syncthreads();
+    // rank sort + exclusive prefix sum of the item counts in one pass over the other requests
+    for (int r = threadIdx.x; r < B; r += blockDim.x) {
+        int c;
+        const int s = get(r, c);
+        const int64_t key = (int64_t)s * (2 * (int64_t)c + s);      // ~ number of (row, key) pairs
+        const int items = (s + 2 * tpt - 1) / (2 * tpt) * Hkv;
+        int64_t off = 0;
+        for (int q = 0; q < B; ++q) {
+            int cq;
+            const int sq = get(q, cq);
+            const int64_t kq = (int64_t)sq * (2 * (int64_t)cq + sq);
+            if (kq > key || (kq == key && q < r)) off += (sq + 2 * tpt - 1) / (2 * tpt) * Hkv;
+        }
+        if (off + items > max_items) {                                // cannot happen for the bound the host computes from B, T
+            atomicOr(&s_err, 2);
+            off = -1;
+        } else {
+            atomicAdd(&s_total, items);
+        }
+        if (in_smem) {
+            s_off[r] = (int)off;
+        } else if (off >= 0) {                                        // large batches: the owning thread writes its items
+            int4* dst = reinterpret_cast<int4*>(work) + 2 + 2 * off;
+            const int npair = (s + 2 * tpt - 1) / (2 * tpt);
+            for (int i = 0; i < npair * Hkv; ++i) {
+                const int kvh = i / npair, t = npair - 1 - i % npair;
+                const int tok0 = t * 2 * tpt;
+                const int64_t q_off = ((int64_t)cu[r] * Hq + (int64_t)kvh * s * g) * D + (int64_t)t * 2 * R * D;   // elements
+                dst[2 * i] = make_int4(c + tok0, min(tpt, s - tok0), max(0, min(tpt, s - tok0 - tpt)), cu[r] + tok0);
+                dst[2 * i + 1] = make_int4(r, kvh, (int)(q_off / 8), 0);
+            }
+        }
+    }
+    __syncthreads();
+    if (in_smem) {
+        // one warp per request, lanes over its items
+        const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+        for (int r = warp; r < B; r += blockDim.x / 32) {
+            const int s = s_s[r], c = s_c[r], off = s_off[r];
+            if (off < 0) continue;
+            const int q_begin = cu[r];
+            int4* dst = reinterpret_cast<int4*>(work) + 2 + 2 * (int64_t)off;
+            const int npair = (s + 2 * tpt - 1) / (2 * tpt);
+            for (int i = lane; i < npair * Hkv; i += 32) {
+                const int kvh = i / npair, t = npair - 1 - i % npair;
+                const int tok0 = t * 2 * tpt;
+                const int64_t q_off = ((int64_t)q_begin * Hq + (int64_t)kvh * s * g) * D + (int64_t)t * 2 * R * D;   // elements
+                dst[2 * i] = make_int4(c + tok0, min(tpt, s - tok0), max(0, min(tpt, s - tok0 - tpt)), q_begin + tok0);
+                dst[2 * i + 1] = make_int4(r, kvh, (int)(q_off / 8), 0);
+            }
+        }
+    }
+    if (threadIdx.x == 0) {
+        work[0] = 0;
+        work[1] = s_err;
+        work[2] = 0;
+        work[3] = s_total;
+    }
 }
 
-int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* tables, int32_t max_blocks,
-                        int32_t* d_work, int64_t num_items, int num_sms, void* stream) {
-    if (num_items == 0) return 0;
+// upper bound on the number of items of a batch with B requests and T suffix rows in total (every request may add one
+// ragged tile pair per kv head)
+int64_t attn_max_items(const cw_config& cfg, int32_t B, int32_t T) {
+    const int g = cfg.num_q_heads / cfg.num_kv_heads;
+    const int tpt2 = 2 * (kTileM / g);
+    return ((int64_t)T / tpt2 + B) * cfg.num_kv_heads;
+}
+
+int64_t attn_work_ints(const cw_config& cfg, int32_t B, int32_t T) {
+    return kWorkInts * (attn_max_items(cfg, B, T) + 1);   // + header
+}
+
+int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* d_cu, const int32_t* d_nc,
+                        const int32_t* d_kv_len, const int32_t* tables, int32_t max_blocks, int32_t B, int32_t T,
+                        int32_t max_q_len, int32_t max_kv_len, int32_t* d_work, int num_sms, void* stream) {
     auto s = static_cast<cudaStream_t>(stream);
+    const int64_t max_items = attn_max_items(cfg, B, T);
+    if (max_items == 0) return 0;
+    attn_schedule_kernel<<<1, 1024, 0, s>>>(d_cu, d_nc, d_kv_len, B, T, cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim,
+                                            max_blocks, cfg.max_position, max_q_len, max_kv_len, d_work, max_items);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return (int)e;
     const float scale_log2 = 1.4426950408889634f / sqrtf((float)cfg.head_dim);
-    const unsigned grid = (unsigned)std::min<int64_t>(num_items, num_sms);
-    cudaError_t e;
+    const unsigned grid = (unsigned)std::min<int64_t>(max_items, num_sms);
 #define CW_LAUNCH_ATTN(DD)                                                                                          \
     do {                                                                                                            \
-        e = cudaFuncSetAttribute(prefill_attn_kernel<DD>, cudaFuncAttributeMaxDynamicSharedMemorySize,              \
-                                 Smem<DD>::kTotal);                                                                 \
-        if (e != cudaSuccess) return (int)e;                                                                        \
+        static bool attr_set = false;                                                                               \
+        if (!attr_set) {                                                                                            \
+            e = cudaFuncSetAttribute(prefill_attn_kernel<DD>, cudaFuncAttributeMaxDynamicSharedMemorySize,          \
+                                     Smem<DD>::kTotal);                                                             \
+            if (e != cudaSuccess) return (int)e;                                                                    \
+            attr_set = true;                                                                                        \
+        }                                                                                                           \
         prefill_attn_kernel<DD><<<grid, kThreads, Smem<DD>::kTotal, s>>>(                                           \
             (const __nv_bfloat16*)q_roped, (__nv_bfloat16*)out, (const __nv_bfloat16*)cfg.k_pool,                   \
-            (const __nv_bfloat16*)cfg.v_pool, tables, max_blocks, (int4*)d_work, (int)num_items,              \
-            cfg.num_q_heads, cfg.num_kv_heads, scale_log2);                                                         \
+            (const __nv_bfloat16*)cfg.v_pool, tables, max_blocks, (int4*)d_work, cfg.num_q_heads,                   \
+            cfg.num_kv_heads, scale_log2);                                                                          \
     } while (0)
     if (cfg.head_dim == 128) CW_LAUNCH_ATTN(128); else CW_LAUNCH_ATTN(64);
 #undef CW_LAUNCH_ATTN

@@ -36,6 +36,7 @@ class Wave:
     nc: np.ndarray                       # int32 [B]
     tables: np.ndarray                   # int32 [B, max_blocks]
     recs: list = field(default_factory=list)
+    reqs: np.ndarray | None = None       # int64 [B] request handles, valid until the wave is released
 
     @property
     def B(self):
@@ -48,6 +49,14 @@ class Wave:
     @property
     def max_blocks(self):
         return int(self.tables.shape[1])
+
+    @property
+    def max_q(self):
+        return int(np.diff(self.cu).max())
+
+    @property
+    def max_kv(self):
+        return int((self.nc + np.diff(self.cu)).max())
 
 
 def make_context(cfg: tracegen.Config, device=None, max_position=None) -> Context:
@@ -102,7 +111,8 @@ class TraceRunner:
             cu = np.zeros(len(recs) + 1, dtype=np.int32)
             cu[1:] = np.cumsum(s)
             wave = Wave([(rec.r, rec.order, rec.n_cached) for rec in recs], cu,
-                        np.array([rec.n_cached for rec in recs], dtype=np.int32), tables, recs)
+                        np.array([rec.n_cached for rec in recs], dtype=np.int32), tables, recs,
+                        np.array([req for req, _ in open_wave], dtype=np.int64))
             if compute:
                 self.prefill_wave(wave, keep_outputs)
             if on_wave is not None:
@@ -144,7 +154,7 @@ class TraceRunner:
         d_cu = torch.from_numpy(wave.cu).to(self.device)
         d_nc = torch.from_numpy(wave.nc).to(self.device)
         d_tables = torch.from_numpy(wave.tables).to(self.device)
-        d_work = torch.empty(max(4, self.ctx.cw_attn_work_ints(wave.cu)), dtype=torch.int32, device=self.device)
+        d_work = torch.empty(self.ctx.cw_attn_work_ints(wave.B, wave.T), dtype=torch.int32, device=self.device)
         return d_cu, d_nc, d_tables, d_work
 
     def prefill_wave(self, wave: Wave, keep_outputs: bool = True):
@@ -153,9 +163,12 @@ class TraceRunner:
         d_cu, d_nc, d_tables, d_work = self.wave_descriptors(wave)
         q_roped, out = torch.empty_like(q), torch.empty_like(q)
         self.ctx.cw_append_kv(q, k, v, q_roped, d_cu, d_nc, d_tables, wave.max_blocks, wave.B, wave.T)
-        self.ctx.cw_prefill_attn(q_roped, out, wave.cu, wave.nc, d_cu, d_nc, d_tables, wave.max_blocks, wave.B,
-                                 wave.T, d_work)
+        s = np.diff(wave.cu)
+        self.ctx.cw_prefill_attn(q_roped, out, d_cu, d_nc, d_tables, wave.max_blocks, wave.B, wave.T,
+                                 int(s.max()), int((wave.nc + s).max()), d_work)
         torch.cuda.synchronize()
+        if int(d_work[1]) != 0:
+            raise RuntimeError("cw_prefill_attn rejected a request descriptor on the device")
         if keep_outputs:
             o = out.view(torch.int16).cpu().numpy().view(np.uint16)
             for b, rec in enumerate(wave.recs):
@@ -185,7 +198,7 @@ def admit_waves(ctx: Context, trace: tracegen.Trace, strategy: str = "greedy", r
                               a["tables"][b, : cfg.blocks_per_req].copy(), int(a["n_cached"][b]), len(waves))
                 for b in range(m)]
         wave = Wave([(rec.r, rec.order, rec.n_cached) for rec in recs], a["cu"][: m + 1].copy(), a["n_cached"][:m].copy(),
-                    a["tables"][:m].copy(), recs)
+                    a["tables"][:m].copy(), recs, a["reqs"][:m].copy())
         if on_wave is not None:
             on_wave(wave)
         ctx.cw_release_batch(a["reqs"][:m])

@@ -1,5 +1,5 @@
 """GPU parity at BASELINE.json's sizes, in the launch configuration bench.py times (wave admission through
-cw_admit_batch, ONE cw_append_kv + ONE cw_prefill_attn per wave), checked on sampled outputs the fp64 oracle computes
+cw_admit_batch, then cw_prefill_requests = ONE cw_append_kv + ONE cw_prefill_attn per wave), checked on sampled outputs the fp64 oracle computes
 row by row.  K/V are keyed by the document prefix (tracegen), so a false cache hit, a wrong block table entry or a block
 evicted too early changes the sampled rows.
 """
@@ -28,13 +28,16 @@ def run_waves_on_gpu(trace, strategy, dev):
     def on_wave(wave):
         rows = tracegen.batch_suffix_qkv(trace, wave.items)
         q, k, v = (torch.from_numpy(x.view(np.int16)).view(torch.bfloat16).to(dev) for x in tracegen.split_qkv(cfg, rows))
-        d_cu, d_nc = torch.from_numpy(wave.cu).to(dev), torch.from_numpy(wave.nc).to(dev)
-        d_tables = torch.from_numpy(wave.tables).to(dev)
         qr, out = torch.empty_like(q), torch.full_like(q, float("nan"))
-        work = torch.empty(max(4, ctx.cw_attn_work_ints(wave.cu)), dtype=torch.int32, device=dev)
-        ctx.cw_append_kv(q, k, v, qr, d_cu, d_nc, d_tables, wave.max_blocks, wave.B, wave.T)
-        ctx.cw_prefill_attn(qr, out, wave.cu, wave.nc, d_cu, d_nc, d_tables, wave.max_blocks, wave.B, wave.T, work)
+        ws = torch.empty(ctx.cw_prefill_requests_ws_bytes(wave.B, wave.T, wave.max_blocks), dtype=torch.uint8, device=dev)
+        ctx.cw_prefill_requests(wave.reqs, q, k, v, qr, out, wave.T, wave.max_blocks, ws)
         torch.cuda.synchronize()
+        hdr = ws[ctx.cw_prefill_requests_work_offset(wave.B, wave.max_blocks):][:16].view(torch.int32).cpu().numpy()
+        assert hdr[1] == 0, "a request descriptor was rejected on the device"
+        # the descriptors the library staged are the ones the admission reported
+        d = ws[: 4 * (2 * wave.B + 1 + wave.B * wave.max_blocks)].view(torch.int32).cpu().numpy()
+        assert np.array_equal(d[: wave.B + 1], wave.cu) and np.array_equal(d[wave.B + 1: 2 * wave.B + 1], wave.nc)
+        assert np.array_equal(d[2 * wave.B + 1:].reshape(wave.B, wave.max_blocks), wave.tables)
         results.append((wave, out.view(torch.int16).cpu().numpy().view(np.uint16)))
 
     admit_waves(ctx, trace, strategy, on_wave=on_wave)

@@ -115,9 +115,13 @@ class Batch:
             self._append([0] * self.B, self.cs)
         qr, cu, nc, d_cu, d_nc, T = self._append(self.cs, self.ns)
         out = torch.full_like(qr, float("nan"))
-        d_work = torch.empty(max(4, self.ctx.cw_attn_work_ints(cu)), dtype=torch.int32, device=self.dev)
-        self.ctx.cw_prefill_attn(qr, out, cu, nc, d_cu, d_nc, self.d_tables, self.max_blocks, self.B, T, d_work)
+        d_work = torch.empty(self.ctx.cw_attn_work_ints(self.B, T), dtype=torch.int32, device=self.dev)
+        d_kv_len = torch.from_numpy(np.asarray(self.ns, dtype=np.int32)).to(self.dev)
+        self.ctx.cw_prefill_attn(qr, out, d_cu, d_nc, self.d_tables, self.max_blocks, self.B, T, max(self.ss), max(self.ns),
+                                 d_work, d_kv_len=d_kv_len)
         torch.cuda.synchronize()
+        self.work_header = d_work[:8].cpu().numpy()          # [claim counter, error flags, fallbacks, items, ...]
+        assert self.work_header[1] == 0, "a request descriptor was rejected on the device"
         return to_bits(qr), to_bits(out), cu
 
     def oracle(self, r):
@@ -181,6 +185,20 @@ def test_attention_matches_oracle(dev, Hq, Hkv, D, cs, ss):
         assert_close_attn(out_bits[cu[r]:cu[r + 1]], b.oracle(r), f"r={r} c={cs[r]} s={ss[r]}")
 
 
+def test_attention_many_small_requests(dev):
+    """2100 requests of 1-3 suffix rows: more requests than the schedule kernel keeps in shared memory (its large-batch
+    path), far more items than CTAs, every item a ragged tile."""
+    rng = np.random.default_rng(21)
+    B = 2100
+    cs = (16 * rng.integers(0, 2, size=B)).tolist()
+    ss = rng.integers(1, 4, size=B).tolist()
+    b = Batch(dev, 2, 1, 64, cs, ss, seed=22)
+    _, out_bits, cu = b.run()
+    assert b.work_header[3] == B                                  # one item per request (1 kv head, < 2 tiles)
+    for r in range(0, B, 7):
+        assert_close_attn(out_bits[cu[r]:cu[r + 1]], b.oracle(r), f"r={r}")
+
+
 def test_attention_constant_v_and_zero_q(dev):
     """V == const => o == const; Q == 0 => o = running mean of V."""
     b = Batch(dev, 8, 2, 128, cs=[0], ss=[300], seed=4)
@@ -197,11 +215,19 @@ def test_empty_batch_and_bad_descriptors(dev):
     z = torch.zeros(4, dtype=torch.int32, device=dev)
     e = torch.empty(0, 2, 64, dtype=torch.bfloat16, device=dev)
     b.ctx.cw_append_kv(e, e, e, e, z, z, z, 1, 0, 0)                           # B = T = 0: OK, no launch
-    b.ctx.cw_prefill_attn(e, e, np.zeros(1, np.int32), np.zeros(0, np.int32), z, z, z, 1, 0, 0, z)
+    b.ctx.cw_prefill_attn(e, e, z, z, z, 1, 0, 0, 0, 0, z)
     q = torch.zeros(20, 2, 64, dtype=torch.bfloat16, device=dev)
-    with pytest.raises(CwError):                                               # n_cached not a multiple of 16
-        b.ctx.cw_prefill_attn(q, torch.empty_like(q), np.array([0, 20], np.int32), np.array([8], np.int32),
-                              z, z, b.d_tables, b.max_blocks, 1, 20, z)
+    with pytest.raises(CwError):                                               # max_kv_len beyond the block table
+        b.ctx.cw_prefill_attn(q, torch.empty_like(q), z, z, b.d_tables, b.max_blocks, 1, 20, 20, 16 * b.max_blocks + 1, z)
+    # descriptors live on the device: an invalid one (n_cached not a multiple of 16) is rejected there — the request
+    # produces no output and the error flag of the work header is set
+    d_cu = torch.tensor([0, 20], dtype=torch.int32, device=dev)
+    d_nc = torch.tensor([8], dtype=torch.int32, device=dev)
+    work = torch.zeros(b.ctx.cw_attn_work_ints(1, 20), dtype=torch.int32, device=dev)
+    out = torch.full_like(q, float("nan"))
+    b.ctx.cw_prefill_attn(q, out, d_cu, d_nc, b.d_tables, b.max_blocks, 1, 20, 20, 20, work)
+    torch.cuda.synchronize()
+    assert int(work[1]) == 1 and int(work[3]) == 0 and bool(torch.isnan(out).all())
     with pytest.raises(CwError):                                               # q_roped aliases q
         b.ctx.cw_append_kv(q, q, q, q, z, z, b.d_tables, b.max_blocks, 1, 20)
 
@@ -271,6 +297,11 @@ def test_attention_growing_maximum_takes_the_exact_path(dev):
         k = tracegen.bf16_bits_to_f64(b.k[r]).astype(np.float32) * ramp[:, None, None]
         b.k[r] = tracegen.f32_to_bf16_bits(k)
     _, out_bits, cu = b.run()
+    assert b.work_header[2] > 0, "the speculative softmax path must have fallen back to the exact one"
+    check_against_rounded_oracle(b, out_bits, cu)
+
+
+def check_against_rounded_oracle(b, out_bits, cu):
     f, rnd = tracegen.bf16_bits_to_f64, lambda x: tracegen.bf16_bits_to_f64(tracegen.f32_to_bf16_bits(x.astype(np.float32)))
     for r in range(b.B):
         n, c = b.ns[r], b.cs[r]
@@ -281,3 +312,85 @@ def test_attention_growing_maximum_takes_the_exact_path(dev):
         got = f(out_bits[cu[r]:cu[r + 1]])
         ref = b.oracle(r)
         assert np.linalg.norm(got - ref) / np.linalg.norm(ref) <= REL_L2
+
+
+@pytest.mark.parametrize("col", [0, 16, 33, 5])
+def test_attention_single_outlier_key_in_a_polynomial_column(dev, col):
+    """One key far down the sequence whose logits exceed the running maximum by > 100 nats for many rows.  Columns 0, 1, 16,
+    17 (mod 32) of a 64-key chunk take exp2 on the FMA pipe (polynomial + exponent splice): without the upper clamp the
+    splice wraps and the row sum stays small, so the overflow check of the speculative path would not fire and the
+    dominant key would be dropped.  The fallback counter proves the exact path ran; outputs are checked as in the
+    growing-maximum test."""
+    b = Batch(dev, 8, 2, 128, cs=[0, 128], ss=[520, 330], seed=13)
+    for r in range(b.B):
+        p = 64 * 5 + col                                        # chunk 5 of the sequence, chosen column
+        k = tracegen.bf16_bits_to_f64(b.k[r]).astype(np.float32)
+        k[p] *= 48.0                                            # logits of this key ~ N(0, 48^2): > +100 for ~2 % of the rows
+        b.k[r] = tracegen.f32_to_bf16_bits(k)
+    _, out_bits, cu = b.run()
+    assert b.work_header[2] > 0, "the speculative softmax path must have fallen back to the exact one"
+    check_against_rounded_oracle(b, out_bits, cu)
+
+
+def test_prefill_attn_returns_before_the_stream_reaches_it(dev):
+    """cw_prefill_attn reads nothing on the host: with a long cw_append_kv queued in front of it the call returns at once
+    (the item list is built by a kernel on the stream), and the host side of the call stays in the tens of microseconds."""
+    import time
+    Hq, Hkv, D, B, s = 32, 8, 128, 48, 2048
+    n = s
+    nblk = n // 16
+    ctx = Context(B * nblk + 8, Hq, Hkv, D, 4, rope_theta=5e5, max_position=n, device=dev)
+    T = B * s
+    g = torch.Generator(device=dev)
+    g.manual_seed(0)
+    q = torch.randn(T, Hq, D, device=dev, dtype=torch.bfloat16, generator=g)
+    k = torch.randn(T, Hkv, D, device=dev, dtype=torch.bfloat16, generator=g)
+    v = torch.randn(T, Hkv, D, device=dev, dtype=torch.bfloat16, generator=g)
+    qr, out = torch.empty_like(q), torch.empty_like(q)
+    tables = torch.arange(B * nblk, dtype=torch.int32, device=dev).reshape(B, nblk).contiguous()
+    d_cu = (torch.arange(B + 1, dtype=torch.int32, device=dev) * s).contiguous()
+    d_nc = torch.zeros(B, dtype=torch.int32, device=dev)
+    work = torch.empty(ctx.cw_attn_work_ints(B, T), dtype=torch.int32, device=dev)
+    host_us = []
+    for it in range(6):
+        torch.cuda.synchronize()
+        for _ in range(4):                                      # ~1.6 ms of HBM-bound work in front of the attention call
+            ctx.cw_append_kv(q, k, v, qr, d_cu, d_nc, tables, nblk, B, T)
+        appended = torch.cuda.Event()
+        appended.record()
+        t0 = time.perf_counter()
+        ctx.cw_prefill_attn(qr, out, d_cu, d_nc, tables, nblk, B, T, s, n, work)
+        t1 = time.perf_counter()
+        still_running = not appended.query()
+        host_us.append(1e6 * (t1 - t0))
+        assert still_running, "cw_prefill_attn returned only after the work queued in front of it had finished"
+    torch.cuda.synchronize()
+    assert int(work[1]) == 0 and int(work[3]) == B * Hkv * (s // (2 * (128 // (Hq // Hkv))))
+    assert np.median(host_us[1:]) < 60.0, host_us               # ctypes marshalling + two launches
+
+
+def test_prefill_requests_equals_separate_calls(dev):
+    """cw_prefill_requests (descriptors taken from the request handles, staged and copied by the library, three launches in
+    one call) is bit-identical to cw_append_kv + cw_prefill_attn with caller-made descriptors, over two waves that share
+    cached blocks."""
+    trace = tracegen.make_trace(tracegen.CONFIGS[1])
+    outs = {}
+    for mode in ("separate", "requests"):
+        run = TraceRunner(trace, "greedy", device=dev)
+        if mode == "requests":
+            ctx = run.ctx
+
+            def prefill_wave(wave, keep_outputs=True, run=run, ctx=ctx):
+                q, k, v = run.wave_inputs(wave)
+                qr, out = torch.empty_like(q), torch.empty_like(q)
+                ws = torch.empty(ctx.cw_prefill_requests_ws_bytes(wave.B, wave.T, wave.max_blocks), dtype=torch.uint8, device=dev)
+                ctx.cw_prefill_requests(wave.reqs, q, k, v, qr, out, wave.T, wave.max_blocks, ws)
+                torch.cuda.synchronize()
+                o = out.view(torch.int16).cpu().numpy().view(np.uint16)
+                for bb, rec in enumerate(wave.recs):
+                    rec.out = o[wave.cu[bb]: wave.cu[bb + 1]]
+            run.prefill_wave = prefill_wave
+        recs = run.run()
+        outs[mode] = [rec.out.copy() for rec in recs]
+    for a, bb in zip(outs["separate"], outs["requests"]):
+        assert np.array_equal(a, bb)

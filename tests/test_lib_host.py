@@ -261,3 +261,24 @@ def test_admit_batch_invalid_arguments():
     assert a["admitted"] == 1 and a["cu"].tolist() == [0, 72]
     with pytest.raises(CwError):
         ctx.cw_release_batch([a["reqs"][0], 12345])
+
+
+def test_admit_batch_invalid_row_leaves_state_untouched():
+    """An invalid row anywhere in the batch (here the LAST one: doc id out of range, then a duplicate) is reported before
+    any request is admitted: no block is pinned or registered and the knowledge tree is unchanged."""
+    from paper_2606_19667_b200 import Context, CwError
+    ctx = Context(64, 2, 1, 64, 4)
+    rng = np.random.default_rng(0)
+    doc_tokens = rng.integers(0, 32000, size=(10, 32), dtype=np.int32)
+    queries = rng.integers(0, 32000, size=(3, 20), dtype=np.int32)
+    before = (ctx.cw_stats(), ctx.cw_free_list())
+    for bad_row in ([0, 1, 10], [4, 4, 5]):
+        ids = np.array([[0, 1, 2], [3, 1, 0], bad_row], dtype=np.int64)
+        with pytest.raises(CwError):
+            ctx.cw_admit_batch(ids, "greedy", doc_tokens, queries)
+        assert (ctx.cw_stats(), ctx.cw_free_list()) == before
+    with pytest.raises(CwError):                                   # unknown arm id
+        ctx.cw_admit_batch(np.array([[0, 1, 2]], dtype=np.int64), 9, doc_tokens, queries[:1])
+    assert (ctx.cw_stats(), ctx.cw_free_list()) == before
+    a = ctx.cw_admit_batch(np.array([[0, 1, 2], [3, 1, 0]], dtype=np.int64), "greedy", doc_tokens, queries[:2])
+    assert a["admitted"] == 2
