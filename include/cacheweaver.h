@@ -206,7 +206,7 @@ int cw_prefill_requests(cw_ctx* ctx, const int64_t* reqs, int32_t B, const void*
  * (device int32 [ceil(n/16)]).  Used by tests and by callers that want the cached KV in a plain layout. */
 int cw_gather_kv(cw_ctx* ctx, const int32_t* d_block_table, int32_t n, void* k_out, void* v_out, void* stream);
 
-/* cw_prefill_host — the same path with HOST buffers (end-to-end entry point).  The batch is cut into up to 8 request
+/* cw_prefill_host — the same path with HOST buffers (end-to-end entry point).  The batch is cut into up to 16 request
  * chunks of about equal token count and pipelined: H2D of chunk i+1 (library-owned copy stream), cw_append_kv +
  * cw_prefill_attn of chunk i (on `stream`, in request order), D2H of chunk i-1 (second copy stream); all of it is
  * enqueued without blocking, then the call waits until everything has completed (`stream` and the copy streams).  q, k, v, out are staged in the

@@ -45,14 +45,15 @@ _lib = None
 
 
 def load_library(build_if_missing: bool = True):
-    """dlopen libcacheweaver.so (building it in-tree with nvcc if it is missing).  Fails loudly otherwise."""
+    """dlopen libcacheweaver.so.  The library is (re)built in-tree with nvcc whenever its source-hash stamp does not match
+    the sources (a missing or stale binary is never used silently).  Fails loudly otherwise."""
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(LIB_PATH):
+    from .build import _stale, build
+    if _stale():
         if not build_if_missing:
-            raise OSError(f"{LIB_PATH} not built; run python -m paper_2606_19667_b200.build")
-        from .build import build
+            raise OSError(f"{LIB_PATH} is missing or older than its sources; run python -m paper_2606_19667_b200.build")
         build()
     lib = C.CDLL(LIB_PATH)
     i32, i64, vp = C.c_int32, C.c_int64, C.c_void_p

@@ -4,6 +4,7 @@
 """
 from __future__ import annotations
 
+import hashlib
 import os
 import subprocess
 import sys
@@ -12,6 +13,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 LIB = os.path.join(PKG, "libcacheweaver.so")
+STAMP = LIB + ".srchash"          # hash of the sources + flags the library was built from (written next to it)
 SOURCES = ["host.cpp", "append_kv.cu", "prefill_attn.cu", "api.cu"]
 HEADERS = ["cw_internal.h", "ptx_sm100.cuh", os.path.join(ROOT, "include", "cacheweaver.h")]
 
@@ -23,26 +25,43 @@ def _nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
+def _flags() -> list:
+    return ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-Xcompiler",
+            "-fPIC,-Wall,-Wno-unused-function"]
+
+
+def source_hash() -> str:
+    """sha256 over the build flags and the contents of every source and header (file names included)."""
+    h = hashlib.sha256(" ".join(_flags()).encode())
+    deps = [os.path.join(CSRC, s) for s in SOURCES] + [x if os.path.isabs(x) else os.path.join(CSRC, x) for x in HEADERS]
+    for d in deps:
+        h.update(os.path.basename(d).encode())
+        with open(d, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()
+
+
 def _stale() -> bool:
-    if not os.path.exists(LIB):
+    """The library is current iff its stamp file holds the hash of today's sources (mtimes are meaningless after a
+    clone or an rsync)."""
+    if not os.path.exists(LIB) or not os.path.exists(STAMP):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, s) for s in SOURCES] + [h if os.path.isabs(h) else os.path.join(CSRC, h) for h in HEADERS]
-    return any(os.path.getmtime(d) > t for d in deps)
+    with open(STAMP) as f:
+        return f.read().strip() != source_hash()
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
-    cmd = [_nvcc(), "-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
-           "-shared", "-Xcompiler", "-fPIC,-Wall,-Wno-unused-function", "-I", os.path.join(ROOT, "include"), "-I", CSRC,
-           "-x", "cu"] + [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB]
-    cmd[1:1] = os.environ.get("CW_NVCC_FLAGS", "").split()      # experiments only (e.g. -DCW_EXP_NOLOAD)
+    cmd = [_nvcc()] + _flags() + ["-I", os.path.join(ROOT, "include"), "-I", CSRC, "-x", "cu"] + \
+          [os.path.join(CSRC, s) for s in SOURCES] + ["-o", LIB]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed:\n" + " ".join(cmd) + "\n" + r.stdout + r.stderr)
+    with open(STAMP, "w") as f:
+        f.write(source_hash() + "\n")
     if verbose:
         print(r.stdout + r.stderr)
     return LIB

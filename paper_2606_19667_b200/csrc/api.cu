@@ -326,7 +326,7 @@ int cw_append_kv(cw_ctx* ctx, const void* q, const void* k, const void* v, void*
     if (T == 0 || B == 0) return CW_OK;
     if (!q || !k || !v || !q_roped || !d_cu || !d_nc || !d_tables || q == q_roped)
         return fail(ctx, CW_ERR_INVALID, "cw_append_kv: null or aliased pointer");
-    int e = cw::launch_append_kv(ctx->cfg, q, k, v, q_roped, d_cu, d_nc, d_tables, max_blocks, B, T, stream);
+    int e = cw::launch_append_kv(ctx->cfg, q, k, v, q_roped, d_cu, d_nc, d_tables, max_blocks, B, T, ctx->num_sms, stream);
     return e ? cuda_fail(ctx, e, "cw_append_kv") : CW_OK;
 }
 
@@ -335,7 +335,7 @@ int cw_gather_kv(cw_ctx* ctx, const int32_t* d_table, int32_t n, void* k_out, vo
     if (n < 0) return fail(ctx, CW_ERR_INVALID, "cw_gather_kv: bad size");
     if (n == 0) return CW_OK;
     if (!d_table || !k_out || !v_out) return fail(ctx, CW_ERR_INVALID, "cw_gather_kv: null pointer");
-    int e = cw::launch_gather_kv(ctx->cfg, d_table, n, k_out, v_out, stream);
+    int e = cw::launch_gather_kv(ctx->cfg, d_table, n, k_out, v_out, ctx->num_sms, stream);
     return e ? cuda_fail(ctx, e, "cw_gather_kv") : CW_OK;
 }
 
@@ -451,7 +451,7 @@ int cw_prefill_requests(cw_ctx* ctx, const int64_t* reqs, int32_t B, const void*
 
 // ---- host-buffer entry point ------------------------------------------------------------------------------
 namespace {
-constexpr int kHostChunks = 8;    // cw_prefill_host pipelines the batch in up to this many request chunks
+constexpr int kHostChunks = 16;   // cw_prefill_host pipelines the batch in up to this many request chunks
 struct WsLayout {
     int64_t q, k, v, qr, out, cu, nc, tables, work, total;
 };

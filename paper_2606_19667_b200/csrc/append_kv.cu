@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(THREADS) append_kv_kernel(
 
 int launch_append_kv(const cw_config& cfg, const void* q, const void* k, const void* v, void* q_roped,
                      const int32_t* cu, const int32_t* ncached, const int32_t* tables, int32_t max_blocks,
-                     int32_t B, int32_t T, void* stream) {
+                     int32_t B, int32_t T, int num_sms, void* stream) {
     if (T == 0) return 0;
     auto s = static_cast<cudaStream_t>(stream);
     // threads per CTA: the multiple of 32 (<= 128) that leaves the fewest idle lanes in the last round over the token's
@@ -127,7 +127,7 @@ int launch_append_kv(const cw_config& cfg, const void* q, const void* k, const v
         if (waste < best_waste) { best_waste = waste; threads = t; }
     }
     const int per_sm = 2048 / threads;
-    int grid = T < 148 * per_sm ? T : 148 * per_sm;
+    const int grid = T < num_sms * per_sm ? T : num_sms * per_sm;
 #define CW_LAUNCH_APPEND(DD, TT)                                                                                \
     append_kv_kernel<DD, TT><<<grid, TT, 0, s>>>(                                                               \
         (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, (__nv_bfloat16*)q_roped,     \
@@ -165,9 +165,9 @@ __global__ void __launch_bounds__(128) gather_kv_kernel(
     }
 }
 
-int launch_gather_kv(const cw_config& cfg, const int32_t* table, int32_t n, void* k_out, void* v_out, void* stream) {
+int launch_gather_kv(const cw_config& cfg, const int32_t* table, int32_t n, void* k_out, void* v_out, int num_sms, void* stream) {
     if (n == 0) return 0;
-    int grid = n < 148 * 8 ? n : 148 * 8;
+    const int grid = n < num_sms * 8 ? n : num_sms * 8;
     auto s = static_cast<cudaStream_t>(stream);
     if (cfg.head_dim == 128)
         gather_kv_kernel<128><<<grid, 128, 0, s>>>((const __nv_bfloat16*)cfg.k_pool, (const __nv_bfloat16*)cfg.v_pool,

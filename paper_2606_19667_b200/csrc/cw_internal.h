@@ -125,8 +125,8 @@ struct cw_ctx {
 namespace cw {
 int launch_append_kv(const cw_config& cfg, const void* q, const void* k, const void* v, void* q_roped,
                      const int32_t* cu, const int32_t* ncached, const int32_t* tables, int32_t max_blocks,
-                     int32_t B, int32_t T, void* stream);
-int launch_gather_kv(const cw_config& cfg, const int32_t* table, int32_t n, void* k_out, void* v_out, void* stream);
+                     int32_t B, int32_t T, int num_sms, void* stream);
+int launch_gather_kv(const cw_config& cfg, const int32_t* table, int32_t n, void* k_out, void* v_out, int num_sms, void* stream);
 // attention: the item list (8 ints per item + an 8-int header) is built on the device by a schedule kernel launched in
 // front of the attention kernel; attn_work_ints is the scratch size for a batch of B requests / T suffix rows
 int64_t attn_max_items(const cw_config& cfg, int32_t B, int32_t T);
