@@ -83,6 +83,11 @@ class BlockManager:
             m += 1
         return m
 
+    def resident_prefix(self, tokens) -> bool:
+        """NEXT-1 peek: are ALL full blocks of this token sequence resident (no cap: the sequence is a document prefix
+        of a longer prompt).  Plain definition again: every leading full block's whole prefix is registered."""
+        return all(k in self.index for k in self._prefix_keys(tokens, len(tokens) // BS))
+
     def lookup(self, tokens):
         n = len(tokens)
         if n <= 0:

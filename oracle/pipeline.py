@@ -49,7 +49,9 @@ def attention_flops(Hq, D, n, c):
 
 def run_trace(trace, strategy: str = "greedy", compute: bool = True, requests=None, sample_rows=None):
     """strategy: 'greedy' (Algorithm 1) | 'retrieval' (identity, the comparison arm PAPER.md:155) | 'sorted' | 'recency' |
-    'exhaustive' (the arms of Table 4, oracle/strategies.py).
+    'exhaustive' (the arms of Table 4, oracle/strategies.py) | 'greedy_feedback' (Algorithm 1 + stale marking from the
+    engine's actual match) | 'greedy_resident' (Algorithm 1 confirmed by peeks on the real index,
+    PAPER.md:314) — the NEXT-1 arms of oracle/ordering.py.
     compute=False does the host path only (order / lookup / tables).
     """
     cfg = trace.cfg
@@ -80,8 +82,10 @@ def run_trace(trace, strategy: str = "greedy", compute: bool = True, requests=No
     while i < len(todo):
         r = todo[i]
         D = trace.retrieval[r]
-        if strategy == "greedy":
+        if strategy in ("greedy", "greedy_feedback"):
             O, depth = tree.order(D)
+        elif strategy == "greedy_resident":
+            O, depth = tree.order_resident(D, lambda docs: bm.resident_prefix(tracegen.doc_prefix_tokens(trace, docs)))
         elif strategy == "retrieval":
             O, depth = list(D), tree.ell(D)
         elif strategy == "sorted":
@@ -103,6 +107,8 @@ def run_trace(trace, strategy: str = "greedy", compute: bool = True, requests=No
                 raise
             close_wave()
             continue                        # retry the same request in the next wave (order() is pure)
+        if strategy in ("greedy_feedback", "greedy_resident"):
+            tree.feedback(O, depth, tracegen.docs_within(trace, O, c))
         tree.observe(O)
         recency.observe(O)
         rr = RequestResult(r, O, depth, tokens, table, c, wave)

@@ -135,6 +135,18 @@ def assemble_prompt(trace: Trace, r: int, order) -> np.ndarray:
     return np.ascontiguousarray(np.concatenate(parts), dtype=np.int32)
 
 
+def doc_prefix_tokens(trace: Trace, docs) -> np.ndarray:
+    """tokens of the prompt prefix made of the leading documents `docs` (no query): what a residency peek looks up."""
+    if len(docs) == 0:
+        return np.zeros(0, dtype=np.int32)
+    return np.ascontiguousarray(np.concatenate([trace.doc_tokens[d] for d in docs]), dtype=np.int32)
+
+
+def docs_within(trace: Trace, order, n_tokens: int) -> int:
+    """number of leading documents of `order` that lie entirely inside the first n_tokens prompt tokens."""
+    return min(len(order), int(n_tokens) // trace.cfg.doc_len)
+
+
 def f32_to_bf16_bits(x: np.ndarray) -> np.ndarray:
     """float32 -> bf16 bit pattern (uint16), round-to-nearest-even.  Input conversion only."""
     u = np.ascontiguousarray(x, dtype=np.float32).view(np.uint32)
