@@ -60,6 +60,12 @@ typedef struct {
     int64_t order_probes;    /* child probes of the last cw_order call (<= k(k+1)/2)          */
     int64_t free_blocks;     /* current length of the LRU free list                                         */
     int64_t seq;             /* number of cw_observe calls so far                                           */
+    /* predicted vs actual reusable prefix ("the trie can predict reuse for a path whose blocks were already
+     * evicted"), summed over the requests admitted by cw_admit_batch and the calls of cw_feedback since cw_create/cw_reset: */
+    int64_t predicted_prefix_docs;   /* sum of l(O,T)                                                        */
+    int64_t actual_prefix_docs;      /* sum of the documents lying entirely inside the matched tokens        */
+    int64_t over_predicted_docs;     /* sum of max(0, predicted - actual)                                    */
+    int64_t stale_marks;             /* trie nodes marked stale (cw_mark_stale, cw_feedback, the residency-aware arm)  */
 } cw_stats_t;
 
 /* ---- lifetime ---------------------------------------------------------------------------------------- */
@@ -107,10 +113,31 @@ int cw_observe(cw_ctx* ctx, const int64_t* ordered_doc_ids, int32_t k);
  *   CW_ARM_EXHAUSTIVE of all k! orders (k <= 8) the one whose prompt matches the most resident blocks (peek lookups on
  *                     the real block index); first maximiser in lexicographic order of retrieval-rank indices.  Needs the
  *                     tokens: doc_tokens [num_docs, doc_len], query_tokens [q_len] (HOST; may be NULL for the other arms).
- * out_order[k] (host); *out_pred_prefix_docs = l(O,T) of the chosen order (may be NULL).  Pure: no state change. */
-enum { CW_ARM_RETRIEVAL = 0, CW_ARM_GREEDY = 1, CW_ARM_SORTED = 2, CW_ARM_RECENCY = 3, CW_ARM_EXHAUSTIVE = 4 };
+ * out_order[k] (host); *out_pred_prefix_docs = l(O,T) of the chosen order (may be NULL).  Pure: no state change (except
+ * CW_ARM_GREEDY_RESIDENT, below).
+ *   CW_ARM_GREEDY_FEEDBACK  Algorithm 1; inside cw_admit_batch the engine's answer is fed back after every lookup
+ *                     (cw_feedback): NEXT-1, PAPER.md:129-141 with the direct cache-state signal instead of TTFT
+ *   CW_ARM_GREEDY_RESIDENT  Algorithm 1 whose line 6 also asks the block index whether the prefix O + [d] is resident
+ *                     (an incremental peek: every full 16-token block completed by the documents placed so far plus d);
+ *                     a recency-cached child that is not resident is marked stale and the scan goes on.  Needs doc_tokens.
+ *                     NOT pure: it marks trie nodes stale (it never changes the block manager).  PAPER.md:314. */
+enum { CW_ARM_RETRIEVAL = 0, CW_ARM_GREEDY = 1, CW_ARM_SORTED = 2, CW_ARM_RECENCY = 3, CW_ARM_EXHAUSTIVE = 4,
+       CW_ARM_GREEDY_FEEDBACK = 5, CW_ARM_GREEDY_RESIDENT = 6 };
 int cw_order_arm(cw_ctx* ctx, int32_t arm, const int64_t* doc_ids, int32_t k, const int32_t* doc_tokens, int32_t num_docs,
                  int32_t doc_len, const int32_t* query_tokens, int32_t q_len, int64_t* out_order, int32_t* out_pred_prefix_docs);
+
+/* Cache-state feedback ("when the trie predicts a long reusable prefix but the
+ * observed TTFT stays close to a cold request, the supposed cached path is probably gone, so we mark it stale and stop
+ * relying on it"; here the engine's own answer replaces the TTFT heuristic).  Reading:
+ *   cw_mark_stale: the document prefix order[0..resident_docs-1] was resident, order[0..resident_docs] was not: the trie
+ *     node at depth resident_docs+1 on that path gets stale_epoch = seq (no-op if the path does not exist).  A node is
+ *     usable iff it is recency-cached AND it was served after the latest stale mark on itself or on any node above it
+ *     on the walk — blocks are chained to their prefix and released deepest-first, so what hangs below an evicted
+ *     prefix is gone as well.  cw_observe re-stamps the served path, which makes exactly that path usable again.
+ *   cw_feedback(order, predicted, actual): if predicted > actual -> cw_mark_stale(order, actual); both also feed the
+ *     predicted-vs-actual counters of cw_stats.  Call it after cw_lookup and before cw_observe. */
+int cw_mark_stale(cw_ctx* ctx, const int64_t* order, int32_t k, int32_t resident_docs);
+int cw_feedback(cw_ctx* ctx, const int64_t* order, int32_t k, int32_t predicted_docs, int32_t actual_docs);
 
 /* ---- prefix cache, host (PAPER.md:33 chained block hashes; PAPER.md:129 block eviction) -------------- */
 /* chain[i] = FNV1a64(LE64(chain[i-1]) || 16 x LE32(token)), chain[-1] = hash_salt, i < floor(n/16). */
@@ -129,7 +156,8 @@ int cw_release(cw_ctx* ctx, int64_t req);
 int cw_reset(cw_ctx* ctx);
 /* Admission of a wave in ONE call: steps a1..a6 (+a2) for requests r = 0..B-1, in order (DESIGN.md reading
  * "requests of a batch are admitted sequentially on the host"):
- *     O_r = cw_order_arm(arm = reorder, doc_ids[r])      (0 = retrieval order, 1 = Algorithm 1, 2.. = the other arms)
+ *     O_r = cw_order_arm(arm = reorder, doc_ids[r])      (0 = retrieval order, 1 = Algorithm 1, 2.. = the other arms;
+ *                                                          arms 5 and 6 also call cw_feedback after the lookup)
  *     tokens = doc_tokens[O_r[0]] || ... || doc_tokens[O_r[k-1]] || query_tokens[r];   (prompt assembly)
  *     (req, table, n_cached) = cw_lookup(tokens);  cw_observe(O_r)
  * All pointers HOST.  doc_ids [B,k] in retrieval rank; doc_tokens [num_docs, doc_len]; query_tokens [B, q_len];

@@ -15,7 +15,8 @@ LIB_PATH = os.path.join(_PKG, "libcacheweaver.so")
 
 CW_OK, CW_ERR_INVALID, CW_ERR_NO_SPACE, CW_ERR_BAD_HANDLE, CW_ERR_CUDA = 0, -1, -2, -3, -4
 BLOCK_SIZE = 16
-ARMS = {"retrieval": 0, "greedy": 1, "sorted": 2, "recency": 3, "exhaustive": 4}     # CW_ARM_* (cacheweaver.h)
+ARMS = {"retrieval": 0, "greedy": 1, "sorted": 2, "recency": 3, "exhaustive": 4,      # CW_ARM_* (cacheweaver.h)
+        "greedy_feedback": 5, "greedy_resident": 6}
 
 
 class CwConfig(C.Structure):
@@ -28,7 +29,8 @@ class CwConfig(C.Structure):
 
 class CwStats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("requests", "hit_blocks", "miss_blocks", "evictions", "trie_nodes",
-                                          "order_probes", "free_blocks", "seq")]
+                                          "order_probes", "free_blocks", "seq", "predicted_prefix_docs",
+                                          "actual_prefix_docs", "over_predicted_docs", "stale_marks")]
 
 
 class CwError(RuntimeError):
@@ -71,6 +73,8 @@ def load_library(build_if_missing: bool = True):
         "cw_predict": (C.c_int, [vp, p(i64), i32, p(i32)]),
         "cw_order_arm": (C.c_int, [vp, i32, p(i64), i32, p(i32), i32, i32, p(i32), i32, p(i64), p(i32)]),
         "cw_observe": (C.c_int, [vp, p(i64), i32]),
+        "cw_mark_stale": (C.c_int, [vp, p(i64), i32, i32]),
+        "cw_feedback": (C.c_int, [vp, p(i64), i32, i32, i32]),
         "cw_hash_chain": (C.c_int, [vp, p(i32), i32, p(C.c_uint64)]),
         "cw_lookup": (C.c_int, [vp, p(i32), i32, i32, p(i64), p(i32), p(i32)]),
         "cw_release": (C.c_int, [vp, i64]),
@@ -97,7 +101,7 @@ def load_library(build_if_missing: bool = True):
 
 
 EXPORTS = ["cw_create", "cw_destroy", "cw_strerror", "cw_last_error", "cw_stats", "cw_pool_bytes", "cw_pool_offset", "cw_q_roped_offset",
-           "cw_order", "cw_predict", "cw_order_arm", "cw_observe", "cw_hash_chain", "cw_lookup", "cw_release", "cw_free_list",
+           "cw_order", "cw_predict", "cw_order_arm", "cw_observe", "cw_mark_stale", "cw_feedback", "cw_hash_chain", "cw_lookup", "cw_release", "cw_free_list",
            "cw_reset", "cw_admit_batch", "cw_release_batch",
            "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_prefill_requests_ws_bytes",
            "cw_prefill_requests_work_offset", "cw_prefill_requests", "cw_gather_kv", "cw_prefill_host_ws_bytes",
@@ -198,6 +202,14 @@ class Context:
     def cw_observe(self, order):
         d = np.ascontiguousarray(order, dtype=np.int64)
         self._check(self.lib.cw_observe(self.h, _i64p(d), len(d)))
+
+    def cw_mark_stale(self, order, resident_docs):
+        d = np.ascontiguousarray(order, dtype=np.int64)
+        self._check(self.lib.cw_mark_stale(self.h, _i64p(d), len(d), int(resident_docs)))
+
+    def cw_feedback(self, order, predicted_docs, actual_docs):
+        d = np.ascontiguousarray(order, dtype=np.int64)
+        self._check(self.lib.cw_feedback(self.h, _i64p(d), len(d), int(predicted_docs), int(actual_docs)))
 
     # ---- prefix cache ----
     def cw_hash_chain(self, tokens):

@@ -129,6 +129,10 @@ int cw_stats(cw_ctx* ctx, cw_stats_t* o) {
     o->order_probes = ctx->tree->probes();
     o->free_blocks = ctx->blocks->free_count();
     o->seq = ctx->tree->seq();
+    o->predicted_prefix_docs = ctx->pred_docs;
+    o->actual_prefix_docs = ctx->actual_docs;
+    o->over_predicted_docs = ctx->over_pred_docs;
+    o->stale_marks = ctx->tree->stale_marks();
     return CW_OK;
 }
 
@@ -166,13 +170,40 @@ int cw_observe(cw_ctx* ctx, const int64_t* ordered, int32_t k) {
     return CW_OK;
 }
 
+int cw_mark_stale(cw_ctx* ctx, const int64_t* order, int32_t k, int32_t resident_docs) {
+    if (!ctx || k < 0 || (k > 0 && !order) || resident_docs < 0) return fail(ctx, CW_ERR_INVALID, "cw_mark_stale: bad argument");
+    ctx->tree->mark_stale(order, k, resident_docs);
+    return CW_OK;
+}
+
+int cw_feedback(cw_ctx* ctx, const int64_t* order, int32_t k, int32_t predicted_docs, int32_t actual_docs) {
+    if (!ctx || k < 0 || (k > 0 && !order) || predicted_docs < 0 || actual_docs < 0)
+        return fail(ctx, CW_ERR_INVALID, "cw_feedback: bad argument");
+    if (predicted_docs > actual_docs) ctx->tree->mark_stale(order, k, actual_docs);
+    ctx->pred_docs += predicted_docs;
+    ctx->actual_docs += actual_docs;
+    ctx->over_pred_docs += std::max(0, predicted_docs - actual_docs);
+    return CW_OK;
+}
+
 int cw_order_arm(cw_ctx* ctx, int32_t arm, const int64_t* doc_ids, int32_t k, const int32_t* doc_tokens, int32_t num_docs,
                  int32_t doc_len, const int32_t* query_tokens, int32_t q_len, int64_t* out_order, int32_t* out_pred) {
-    if (!ctx || k < 0 || (k > 0 && (!doc_ids || !out_order)) || arm < CW_ARM_RETRIEVAL || arm > CW_ARM_EXHAUSTIVE)
+    if (!ctx || k < 0 || (k > 0 && (!doc_ids || !out_order)) || arm < CW_ARM_RETRIEVAL || arm > CW_ARM_GREEDY_RESIDENT)
         return fail(ctx, CW_ERR_INVALID, "cw_order_arm: bad argument");
     if (has_duplicates(doc_ids, k)) return fail(ctx, CW_ERR_INVALID, "cw_order_arm: duplicate document id");
-    if (arm == CW_ARM_GREEDY) {
+    if (arm == CW_ARM_GREEDY || arm == CW_ARM_GREEDY_FEEDBACK) {
         ctx->tree->order(doc_ids, k, out_order);
+    } else if (arm == CW_ARM_GREEDY_RESIDENT) {
+        if (doc_len < 0 || (k > 0 && !doc_tokens))
+            return fail(ctx, CW_ERR_INVALID, "cw_order_arm: the residency-aware arm needs the document tokens");
+        for (int i = 0; i < k; ++i)
+            if (doc_ids[i] < 0 || doc_ids[i] >= num_docs) return fail(ctx, CW_ERR_INVALID, "cw_order_arm: doc id out of range");
+        // peek on the real block index, incremental over the confirmed document prefix
+        cw::BlockManager::Probe probe = ctx->blocks->probe_begin();
+        const std::function<bool(const int64_t*, int, int64_t)> resident = [&](const int64_t*, int, int64_t d) {
+            return ctx->blocks->probe_extend(probe, doc_tokens + (size_t)d * doc_len, doc_len);
+        };
+        ctx->tree->order(doc_ids, k, out_order, &resident);
     } else if (arm == CW_ARM_RETRIEVAL) {
         std::memcpy(out_order, doc_ids, sizeof(int64_t) * (size_t)k);
     } else if (arm == CW_ARM_SORTED) {
@@ -250,6 +281,7 @@ int cw_reset(cw_ctx* ctx) {
     ctx->blocks = new cw::BlockManager(ctx->cfg.num_blocks, ctx->cfg.eager_register != 0, ctx->cfg.hash_salt);
     ctx->last_served.clear();
     ctx->last_error.clear();
+    ctx->pred_docs = ctx->actual_docs = ctx->over_pred_docs = 0;
     return CW_OK;
 }
 
@@ -269,7 +301,7 @@ int cw_admit_batch(cw_ctx* ctx, const int64_t* doc_ids, int32_t B, int32_t k, in
         !out_tables || !out_nc)
         return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: null pointer");
     const int32_t n = (int32_t)n64, nblk = (n + CW_BLOCK_SIZE - 1) / CW_BLOCK_SIZE;
-    if (reorder < CW_ARM_RETRIEVAL || reorder > CW_ARM_EXHAUSTIVE || (reorder == CW_ARM_EXHAUSTIVE && k > 8))
+    if (reorder < CW_ARM_RETRIEVAL || reorder > CW_ARM_GREEDY_RESIDENT || (reorder == CW_ARM_EXHAUSTIVE && k > 8))
         return fail(ctx, CW_ERR_INVALID, "cw_admit_batch: unknown ordering arm (or exhaustive with k > 8)");
     // every row is validated BEFORE anything is admitted: an invalid argument leaves the state untouched
     for (int32_t r = 0; r < B; ++r) {
@@ -295,6 +327,16 @@ int cw_admit_batch(cw_ctx* ctx, const int64_t* doc_ids, int32_t B, int32_t k, in
         if (rc == CW_ERR_NO_SPACE) return CW_OK;
         if (rc != CW_OK) return rc;
         for (int32_t i = nblk; i < max_blocks; ++i) table[i] = 0;
+        {   // predicted vs actual prefix: documents lying entirely inside the cached tokens
+            const int32_t actual = doc_len > 0 ? std::min<int32_t>(k, out_nc[r] / doc_len) : 0;
+            if (reorder == CW_ARM_GREEDY_FEEDBACK || reorder == CW_ARM_GREEDY_RESIDENT) {
+                cw_feedback(ctx, O, k, out_pred[r], actual);
+            } else {
+                ctx->pred_docs += out_pred[r];
+                ctx->actual_docs += actual;
+                ctx->over_pred_docs += std::max(0, out_pred[r] - actual);
+            }
+        }
         ctx->tree->observe(O, k);
         for (int i = 0; i < k; ++i) ctx->last_served[O[i]] = ctx->tree->seq();
         out_cu[r + 1] = out_cu[r] + (n - out_nc[r]);

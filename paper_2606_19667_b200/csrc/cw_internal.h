@@ -1,7 +1,9 @@
 // Internal declarations shared by the host state (host.cpp), the kernels (*.cu) and the C ABI (api.cu).
 // Product code: nothing here is shared with oracle/.
 #pragma once
+#include <algorithm>
 #include <cstdint>
+#include <functional>
 #include <string>
 #include <unordered_map>
 #include <vector>
@@ -29,22 +31,30 @@ struct TrieKeyHash {
 struct TrieNode {
     uint64_t id;
     int64_t last_seq;
+    int64_t stale_epoch;    // seq at which the engine reported this prefix as not resident (0 = never); DESIGN.md §2 NEXT-1
 };
 
 class KnowledgeTree {
   public:
     explicit KnowledgeTree(int64_t window) : H_(window) {}
-    // Algorithm 1.  Returns depth l(O,T).
-    int order(const int64_t* D, int k, int64_t* O);
+    // Algorithm 1.  Returns depth l(O,T).  `resident` (optional, NEXT-1): asked for every recency-cached
+    // child whether the document prefix O[0..m-1] + d is really resident (m = documents placed so far); a child that is
+    // not is marked stale and the scan goes on.
+    int order(const int64_t* D, int k, int64_t* O, const std::function<bool(const int64_t* O, int m, int64_t d)>* resident = nullptr);
     int predict(const int64_t* O, int k) const;
     void observe(const int64_t* O, int k);
+    // the prefix O[0..a-1] was resident, O[0..a] was not: the node at depth a+1 is marked stale (no-op if it does not exist)
+    void mark_stale(const int64_t* O, int k, int a);
     int64_t nodes() const { return (int64_t)map_.size(); }
     int64_t probes() const { return probes_; }
     int64_t seq() const { return seq_; }
+    int64_t stale_marks() const { return marks_; }
 
   private:
     const TrieNode* child(uint64_t parent, int64_t doc) const;
     bool cached(const TrieNode* n) const { return seq_ - n->last_seq < H_; }
+    // usable: cached by recency and served after the latest stale mark on itself or above it on the walk (floor)
+    bool usable(const TrieNode* n, int64_t floor) const { return cached(n) && n->last_seq > std::max(floor, n->stale_epoch); }
     void prune();
     std::unordered_map<TrieKey, TrieNode, TrieKeyHash> map_;
     int64_t H_;
@@ -52,6 +62,7 @@ class KnowledgeTree {
     int64_t last_prune_ = 0;
     uint64_t next_id_ = 1;  // 0 = root
     int64_t probes_ = 0;
+    int64_t marks_ = 0;     // nodes marked stale so far
 };
 
 // ---- paged KV block manager (reading c3) --------------------------------
@@ -67,6 +78,16 @@ class BlockManager {
     BlockManager(int32_t num_blocks, bool eager, uint64_t salt);
     void chain(const int32_t* tokens, int32_t n, std::vector<uint64_t>& out) const;
     int32_t match(const std::vector<uint64_t>& chain, int32_t n) const;
+    // NEXT-1 peek, incremental over a growing document prefix: state = (hash of the last full block, tokens of the
+    // pending partial block).  extend() appends tokens; it returns false and leaves the state unchanged unless every
+    // full block completed by them is resident.
+    struct Probe {
+        uint64_t parent;
+        int32_t pending[CW_BLOCK_SIZE];
+        int32_t n_pending;
+    };
+    Probe probe_begin() const { return Probe{salt_, {0}, 0}; }
+    bool probe_extend(Probe& p, const int32_t* tokens, int32_t n) const;
     // returns CW_OK / CW_ERR_NO_SPACE
     int lookup(const int32_t* tokens, int32_t n, int64_t* req, int32_t* table, int32_t* n_cached);
     int release(int64_t req);
@@ -105,6 +126,8 @@ struct cw_ctx {
     int num_sms;
     // comparison arms (cw_order_arm): index of the last cw_observe call whose order contained the document
     std::unordered_map<int64_t, int64_t> last_served;
+    // predicted-vs-actual prefix statistics, accumulated by cw_admit_batch / cw_feedback
+    int64_t pred_docs = 0, actual_docs = 0, over_pred_docs = 0;
     // cw_prefill_host pipeline: copy streams and per-chunk events (created on first use, destroyed with the context)
     void* copy_in_stream = nullptr;
     void* copy_out_stream = nullptr;

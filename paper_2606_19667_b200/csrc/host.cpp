@@ -16,23 +16,30 @@ const TrieNode* KnowledgeTree::child(uint64_t parent, int64_t doc) const {
 
 // Algorithm 1.  R is kept as an index list in retrieval rank; "for each d in R" scans it in that order and takes
 // the first cached child (DESIGN.md reading: D is given in retrieval rank).
-int KnowledgeTree::order(const int64_t* D, int k, int64_t* O) {
+int KnowledgeTree::order(const int64_t* D, int k, int64_t* O,
+                         const std::function<bool(const int64_t* O, int m, int64_t d)>* resident) {
     std::vector<int64_t> R(D, D + k);                 // line 1: O <- [], R <- D, node <- root
     uint64_t node = 0;
+    int64_t floor = 0;
     int n_out = 0;
     probes_ = 0;
     while (!R.empty()) {                              // line 2
         bool found = false;                           // line 3
         for (size_t i = 0; i < R.size(); ++i) {       // line 4
             ++probes_;
-            const TrieNode* c = child(node, R[i]);    // line 5
-            if (c && cached(c)) {                     // line 6
-                O[n_out++] = R[i];                    // line 7: append d to O, remove d from R
-                R.erase(R.begin() + (long)i);
-                node = c->id;                         // line 8
-                found = true;
-                break;
+            auto it = map_.find(TrieKey{node, R[i]}); // line 5
+            if (it == map_.end() || !usable(&it->second, floor)) continue;   // line 6
+            if (resident && !(*resident)(O, n_out, R[i])) {
+                it->second.stale_epoch = seq_;        // predicted resident, really gone: stop relying on it
+                ++marks_;
+                continue;
             }
+            O[n_out++] = R[i];                        // line 7: append d to O, remove d from R
+            R.erase(R.begin() + (long)i);
+            node = it->second.id;                     // line 8
+            floor = std::max(floor, it->second.stale_epoch);
+            found = true;
+            break;
         }
         if (!found) {                                 // lines 11-13: remaining R in retrieval-rank order
             for (int64_t d : R) O[n_out++] = d;
@@ -44,13 +51,29 @@ int KnowledgeTree::order(const int64_t* D, int k, int64_t* O) {
 
 int KnowledgeTree::predict(const int64_t* O, int k) const {
     uint64_t node = 0;
+    int64_t floor = 0;
     int m = 0;
     for (; m < k; ++m) {
         const TrieNode* c = child(node, O[m]);
-        if (!c || !cached(c)) break;
+        if (!c || !usable(c, floor)) break;
         node = c->id;
+        floor = std::max(floor, c->stale_epoch);
     }
     return m;
+}
+
+void KnowledgeTree::mark_stale(const int64_t* O, int k, int a) {
+    if (a < 0 || a >= k) return;
+    uint64_t node = 0;
+    for (int i = 0; i <= a; ++i) {
+        auto it = map_.find(TrieKey{node, O[i]});
+        if (it == map_.end()) return;
+        if (i == a) {
+            it->second.stale_epoch = seq_;
+            ++marks_;
+        }
+        node = it->second.id;
+    }
 }
 
 void KnowledgeTree::observe(const int64_t* O, int k) {
@@ -59,7 +82,7 @@ void KnowledgeTree::observe(const int64_t* O, int k) {
     for (int i = 0; i < k; ++i) {
         TrieKey key{node, O[i]};
         auto it = map_.find(key);
-        if (it == map_.end()) it = map_.emplace(key, TrieNode{next_id_++, seq_}).first;
+        if (it == map_.end()) it = map_.emplace(key, TrieNode{next_id_++, seq_, 0}).first;
         it->second.last_seq = seq_;
         node = it->second.id;
     }
@@ -100,20 +123,36 @@ void BlockManager::push_tail(int32_t b) {
     ++free_count_;
 }
 
+static inline uint64_t block_hash(uint64_t parent, const int32_t* tokens) {
+    uint64_t h = 0xCBF29CE484222325ull;
+    for (int b = 0; b < 8; ++b) h = fnv1a_step(h, (uint8_t)(parent >> (8 * b)));
+    for (int t = 0; t < CW_BLOCK_SIZE; ++t) {
+        uint32_t tok = (uint32_t)tokens[t];
+        for (int b = 0; b < 4; ++b) h = fnv1a_step(h, (uint8_t)(tok >> (8 * b)));
+    }
+    return h;
+}
+
 // h_i = FNV1a64(LE64(h_{i-1}) || LE32(tok[16i]) ... LE32(tok[16i+15])), h_{-1} = salt  (DESIGN.md c2)
 void BlockManager::chain(const int32_t* tokens, int32_t n, std::vector<uint64_t>& out) const {
     int32_t nfull = n / CW_BLOCK_SIZE;
     out.resize((size_t)nfull);
     uint64_t parent = salt_;
-    for (int32_t i = 0; i < nfull; ++i) {
-        uint64_t h = 0xCBF29CE484222325ull;
-        for (int b = 0; b < 8; ++b) h = fnv1a_step(h, (uint8_t)(parent >> (8 * b)));
-        for (int t = 0; t < CW_BLOCK_SIZE; ++t) {
-            uint32_t tok = (uint32_t)tokens[i * CW_BLOCK_SIZE + t];
-            for (int b = 0; b < 4; ++b) h = fnv1a_step(h, (uint8_t)(tok >> (8 * b)));
+    for (int32_t i = 0; i < nfull; ++i) out[(size_t)i] = parent = block_hash(parent, tokens + (size_t)i * CW_BLOCK_SIZE);
+}
+
+bool BlockManager::probe_extend(Probe& p, const int32_t* tokens, int32_t n) const {
+    Probe q = p;
+    for (int32_t i = 0; i < n; ++i) {
+        q.pending[q.n_pending++] = tokens[i];
+        if (q.n_pending == CW_BLOCK_SIZE) {
+            q.parent = block_hash(q.parent, q.pending);
+            if (!index_.count(q.parent)) return false;
+            q.n_pending = 0;
         }
-        out[(size_t)i] = parent = h;
     }
+    p = q;
+    return true;
 }
 
 int32_t BlockManager::match(const std::vector<uint64_t>& ch, int32_t n) const {

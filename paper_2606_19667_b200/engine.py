@@ -84,7 +84,7 @@ class TraceRunner:
     # ---- host path -----------------------------------------------------------------------------------------
     def _admit(self, r):
         D = self.trace.retrieval[r]
-        if self.strategy == "greedy":
+        if self.strategy in ("greedy", "greedy_feedback"):
             O, depth = self.ctx.cw_order(D)
         elif self.strategy == "retrieval":
             O, depth = list(D), self.ctx.cw_predict(D)
@@ -92,6 +92,8 @@ class TraceRunner:
             O, depth = self.ctx.cw_order_arm(self.strategy, D, self.trace.doc_tokens, self.trace.query_tokens[r])
         tokens = tracegen.assemble_prompt(self.trace, r, O)
         req, table, c = self.ctx.cw_lookup(tokens)        # raises NoSpace with state unchanged
+        if self.strategy in ("greedy_feedback", "greedy_resident"):
+            self.ctx.cw_feedback(O, depth, tracegen.docs_within(self.trace, O, c))
         self.ctx.cw_observe(O)
         return req, RequestRecord(r, O, depth, tokens, table, c, len(self.waves))
 

@@ -233,7 +233,8 @@ def test_empty_batch_and_bad_descriptors(dev):
 
 
 # ---- whole path on the BASELINE.json traces ---------------------------------------------------------------
-@pytest.mark.parametrize("strategy", ["greedy", "retrieval"])
+@pytest.mark.parametrize("strategy", ["greedy", "retrieval", "sorted", "recency", "exhaustive", "greedy_feedback",
+                                      "greedy_resident"])
 def test_trace_cfg1_all_rows(dev, strategy):
     trace = tracegen.make_trace(tracegen.CONFIGS[1])
     ref = run_trace(trace, strategy)
@@ -246,6 +247,23 @@ def test_trace_cfg1_all_rows(dev, strategy):
         assert_close_attn(a.out, o.out, f"cfg1 {strategy} r={a.r}")
         # prefix-cached == full recompute of the same ordered prompt
         assert_close_attn(a.out, full_recompute(trace, o)[o.n_cached:], f"cfg1 {strategy} r={a.r} vs full")
+
+
+@pytest.mark.parametrize("strategy", ["greedy", "greedy_feedback", "greedy_resident", "exhaustive"])
+def test_trace_with_eviction_all_rows(dev, strategy):
+    """A pool that holds only ~4 prompts, 30 wave-admitted requests: blocks the trie still believes resident are evicted
+    (PAPER.md:129).  Orders, depths, tables bit-exact and every output row within tolerance, for the plain arm and the
+    NEXT-1 arms (feedback / residency-aware) — a stale block table entry or a false hit changes K/V and fails."""
+    import dataclasses
+    cfg = dataclasses.replace(tracegen.CONFIGS[1], name="evict-gpu", seed=5, n_docs=8, doc_len=32, n_req=30, k=3, n_shared=2,
+                              q_len=20, NB=32, H=16, admission="waves")
+    trace = tracegen.make_trace(cfg)
+    ref = run_trace(trace, strategy)
+    recs = TraceRunner(trace, strategy, device=dev).run()
+    assert ref.evictions > 0 and len(recs) == len(ref.requests)
+    for a, o in zip(recs, ref.requests):
+        assert (a.order, a.depth, a.n_cached, a.table.tolist(), a.wave) == (o.order, o.depth, o.n_cached, list(o.table), o.wave)
+        assert_close_attn(a.out, o.out, f"evict {strategy} r={a.r}")
 
 
 def test_trace_cfg2_first_requests_all_rows(dev):
