@@ -52,11 +52,12 @@ def peaks():
     return {"bf16": 1590.0, "bf16_sustained": 1400.0, "hbm": 6650.0, "source": "fallback (B200_PROFILING.md)"}
 
 
-def traffic_from_profile(kernel):
-    """dram bytes per launch from the committed ncu summary (profiles/traffic.json), else None."""
+def traffic_from_profile(cfg_name, kernel):
+    """dram__bytes_read + dram__bytes_write per launch of `kernel` on configuration `cfg_name`, from the committed ncu
+    capture listed in profiles/traffic.json; None when that configuration was never captured."""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(p):
-        return json.load(open(p)).get(kernel)
+        return json.load(open(p)).get(cfg_name, {}).get(kernel)
     return None
 
 
@@ -110,7 +111,7 @@ class Workload:
     """One configuration, one strategy: seeded trace, resident inputs, and the step function."""
     RING = 4
 
-    def __init__(self, cfg_id, strategy, device, want_e2e=True, device_inputs=False, sequential=False):
+    def __init__(self, cfg_id, strategy, device, want_e2e=True, device_inputs=False, sequential=False, real_waves=0):
         import torch
         from paper_2606_19667_b200.engine import admit_waves, make_context
         self.torch, self.device, self.strategy = torch, device, strategy
@@ -129,7 +130,7 @@ class Workload:
         Bmax = max(w.B for w in self.waves)
         self.inputs, self.host_inputs = [], []
         for wi, w in enumerate(self.waves):
-            if device_inputs:
+            if device_inputs and wi >= real_waves:
                 # timing-only runs of the large configs / the sweep: seeded N(0,1) bf16 drawn on the device (the values do
                 # not change the work; parity at these shapes is covered by tests/test_gpu_full_size.py with tracegen inputs)
                 g = torch.Generator(device=device)
@@ -141,7 +142,7 @@ class Workload:
                 continue
             rows = tracegen.batch_suffix_qkv(trace, w.items, threads=os.cpu_count() or 8)
             qkv = [torch.from_numpy(x.view(np.int16)).view(torch.bfloat16) for x in tracegen.split_qkv(cfg, rows)]
-            if want_e2e:
+            if want_e2e and not device_inputs:
                 self.host_inputs.append([t.pin_memory() for t in qkv] + [torch.empty_like(qkv[0]).pin_memory()])
             dq, dk, dv = (t.to(device) for t in qkv)
             work = torch.empty(self.ctx.cw_attn_work_ints(w.B, w.T), dtype=torch.int32, device=device)
@@ -168,7 +169,7 @@ class Workload:
             self.req_ws = torch.empty(max(self.ctx.cw_prefill_requests_ws_bytes(w.B, w.T, self.max_blocks) for w in self.waves),
                                       dtype=torch.uint8, device=device)
         self.ws = None
-        if want_e2e:
+        if want_e2e and not device_inputs:
             nbytes = max(self.ctx.cw_prefill_host_ws_bytes(w.B, w.T, self.max_blocks) for w in self.waves)
             self.ws = torch.empty(nbytes, dtype=torch.uint8, device=device)
         self.queries = np.ascontiguousarray(trace.query_tokens)
@@ -224,6 +225,22 @@ class Workload:
             self.launches += 3
             lo += B
 
+    def host_admission(self, reps=3):
+        """host path alone (a1-a6 + a9 for every request of the configuration): us per request, and the predicted-vs-actual
+        prefix counters of one pass (cw_stats)."""
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            self.ctx.cw_reset()
+            lo = 0
+            for w in self.waves:
+                st, a = self._admit(lo, w)
+                self.ctx.cw_release_batch(a["reqs"][:w.B])
+                lo += w.B
+        us = (time.perf_counter() - t0) / reps * 1e6 / self.cfg.n_req
+        st = self.ctx.cw_stats()
+        return us, {k: st[k] for k in ("predicted_prefix_docs", "actual_prefix_docs", "over_predicted_docs", "stale_marks",
+                                       "hit_blocks", "evictions")}
+
     def step_e2e(self):
         """host buffers: admission + cw_prefill_host (H2D of q,k,v and descriptors, both kernels, D2H of out)."""
         ctx = self.ctx
@@ -257,7 +274,7 @@ class OracleSample:
 
     def __init__(self, cfg_id, n_req):
         from oracle.pipeline import run_trace
-        self.cfg = cfg = tracegen.CONFIGS[cfg_id]
+        self.cfg = cfg = tracegen.CONFIGS[cfg_id] if isinstance(cfg_id, int) else cfg_id
         self.trace = tracegen.make_trace(cfg)
         self.reqs = list(range(min(n_req, cfg.n_req)))
         dry = run_trace(self.trace, "greedy", compute=False, requests=self.reqs)
@@ -295,7 +312,7 @@ def run_reference(args):
     rank, _, world = dist_env()
     if rank != 0:
         return
-    sample = OracleSample(args.config, args.oracle_requests)
+    sample = OracleSample(select_config(args), args.oracle_requests)
     for _ in range(args.warmup):
         sample.run()
     times = [sample.run() for _ in range(args.steps)]
@@ -356,11 +373,19 @@ def run_ours(args):
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device(device))
     pk = peaks()
-    wl = Workload(args.config, "greedy", device, want_e2e=not args.device_inputs, device_inputs=args.device_inputs)
+    cfg_sel = select_config(args)
+    wl = Workload(cfg_sel, args.arm, device, want_e2e=not args.device_inputs, device_inputs=args.device_inputs,
+                  real_waves=args.real_waves)
     cfg = wl.cfg
 
     for _ in range(args.warmup):
         wl.step()
+    if args.seconds > 0:       # long run: as many steps as fit the requested wall time (sustained clocks / power cap)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        wl.step()
+        torch.cuda.synchronize()
+        args.steps = max(args.steps, int(args.seconds / max(1e-6, time.perf_counter() - t0)))
     wl.launches = 0
     events = []
     with ClockSampler(local) as clk:
@@ -389,11 +414,14 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     # second half of the metric: batch prefill ms, greedy vs retrieval order (same trace, fresh context)
-    prefill = {"greedy": {"ms": app_ms + attn_ms, "append_ms": app_ms, "attn_ms": attn_ms, "suffix_tokens": wl.T,
-                          "hit_blocks": wl.hit_blocks, "attn_flops": wl.flops}}
+    host_us, pred = wl.host_admission()
+    prefill = {args.arm: {"ms": app_ms + attn_ms, "append_ms": app_ms, "attn_ms": attn_ms, "suffix_tokens": wl.T,
+                          "hit_blocks": wl.hit_blocks, "attn_flops": wl.flops, "waves": len(wl.waves),
+                          "predicted_prefix_docs": pred["predicted_prefix_docs"], "actual_prefix_docs": pred["actual_prefix_docs"],
+                          "over_predicted_docs": pred["over_predicted_docs"], "stale_marks": pred["stale_marks"]}}
     if not args.skip_retrieval:
         del wl.host_inputs, wl.ws
-        wr = Workload(args.config, "retrieval", device, want_e2e=False, device_inputs=args.device_inputs)
+        wr = Workload(cfg_sel, "retrieval", device, want_e2e=False, device_inputs=args.device_inputs, real_waves=args.real_waves)
         for _ in range(args.warmup):
             wr.step()
         ev = []
@@ -401,14 +429,14 @@ def run_ours(args):
         r_app = sum(e[0].elapsed_time(e[1]) for e in ev) / args.steps
         r_attn = sum(e[1].elapsed_time(e[2]) for e in ev) / args.steps
         prefill["retrieval"] = {"ms": r_app + r_attn, "append_ms": r_app, "attn_ms": r_attn, "suffix_tokens": wr.T,
-                                "hit_blocks": wr.hit_blocks, "attn_flops": wr.flops}
-        prefill["ratio_measured"] = prefill["greedy"]["ms"] / prefill["retrieval"]["ms"]
+                                "hit_blocks": wr.hit_blocks, "attn_flops": wr.flops, "waves": len(wr.waves)}
+        prefill["ratio_measured"] = prefill[args.arm]["ms"] / prefill["retrieval"]["ms"]
         prefill["ratio_predicted_by_flops"] = wl.flops / wr.flops
         del wr
-        if cfg.admission == "sequential":
+        if cfg.admission == "sequential" and not args.skip_per_request:
             # the honest per-request figure: every request admitted, launched (2 kernels) and released
             # on its own — launch-bound on this shape (one request is 5-15 us of tensor work)
-            ws = Workload(args.config, "greedy", device, want_e2e=False, device_inputs=True, sequential=True)
+            ws = Workload(cfg_sel, args.arm, device, want_e2e=False, device_inputs=True, sequential=True)
             for _ in range(args.warmup):
                 ws.step()
             s_ms = timed(torch, ws.step, args.steps, None) / args.steps
@@ -417,9 +445,11 @@ def run_ours(args):
                                                "value_tflops": ws.flops / (s_ms * 1e-3) / 1e12}
             del ws
 
+    if cfg.name.startswith("cfg1"):
+        prefill["arms_cfg1"] = cfg1_four_arms(device)
     cpu = None
     if world == 1 or rank == 0:
-        sample = OracleSample(args.config, args.oracle_requests)
+        sample = OracleSample(cfg_sel, args.oracle_requests)
         t = sample.run()
         desc = f"first {len(sample.reqs)} of {cfg.n_req} requests of {cfg.name}, sequential, greedy order, one pass"
         cpu = {"value": sample.flops / t / 1e12, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle", "sample": desc,
@@ -431,25 +461,84 @@ def run_ours(args):
             "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({cfg.name})", "requests": cfg.n_req,
                        "prompt_tokens": cfg.n, "heads": f"{cfg.Hq}q/{cfg.Hkv}kv x {cfg.D}", "pool_blocks": cfg.NB,
                        "admission": f"one varlen wave per launch ({n_l} wave(s)), eager block registration",
-                       "order": "greedy", "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "order": args.arm, "parallelism": "replicas only" if world > 1 else "1 GPU",
+                       "inputs": ("tracegen activations (keyed by document prefix)" if not args.device_inputs else
+                                  f"tracegen activations for the first {min(args.real_waves, n_l)} wave(s), device-drawn N(0,1) for the rest"),
                        "l2": "inputs larger than L2 (q,k,v,pool >> 126 MB per step); no explicit flush"},
             "pct_of_bf16_peak": 100.0 * value / world / pk["bf16"],
             "clocks": clk.summary(),
             "e2e": ({"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": wl.h2d // e2e_steps,
                      "d2h_bytes_per_step": wl.d2h // e2e_steps, "ms_per_step": ms_e2e, "steps": e2e_steps} if e2e_steps else None),
             "gpu_launches": launches,
+            "host_us_per_request": {"value": host_us, "what": "cw_order + prompt assembly + cw_lookup + cw_observe + cw_release per request "
+                                    "(one cw_admit_batch + cw_release_batch call per wave)", "paper": "66.6 us = order 22.2 + build 44.4 "
+                                    "(Python middleware, PAPER.md:244-251 Table 8; other hardware, context only)"},
             "roofline": {"kernel": "prefill_attn_kernel", "bound": "tensor", "achieved": attn_tflops, "peak": pk["bf16"],
-                         "unit": "TFLOP/s", "frac": attn_tflops / pk["bf16"], "traffic": traffic_from_profile("prefill_attn_kernel"),
+                         "unit": "TFLOP/s", "frac": attn_tflops / pk["bf16"], "traffic": traffic_from_profile(cfg.name, "prefill_attn_kernel"),
+                         "window": "schedule kernel + attention kernel (cw_prefill_attn), CUDA events on the launching stream",
                          "peak_source": pk["source"], "frac_of_sustained": attn_tflops / pk["bf16_sustained"],
                          "flops_per_step": wl.flops, "avg_ms": attn_ms / n_l, "launches_per_step": n_l},
             "roofline_append_kv": {"kernel": "append_kv_kernel", "bound": "hbm", "achieved": app_gbs, "peak": pk["hbm"],
-                                   "unit": "GB/s", "frac": app_gbs / pk["hbm"], "traffic": traffic_from_profile("append_kv_kernel"),
+                                   "unit": "GB/s", "frac": app_gbs / pk["hbm"], "traffic": traffic_from_profile(cfg.name, "append_kv_kernel"),
                                    "bytes_per_step": append_bytes(cfg, wl.T), "avg_ms": app_ms / n_l},
             "batch_prefill": prefill,
             "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
+
+
+def select_config(args):
+    """--config N, with the variants --one-wave (cfg 4 with a pool that holds the whole batch) and
+    --config 3 --k K --overlap P (one cell of the sweep)."""
+    import dataclasses
+    if args.config == 3:
+        return tracegen.config3(args.k, args.overlap)
+    cfg = tracegen.CONFIGS[args.config]
+    if args.one_wave:
+        nb = 1 << (cfg.n_req * cfg.blocks_per_req - 1).bit_length()
+        cfg = dataclasses.replace(cfg, name=cfg.name + f"-onewave-NB{nb}", NB=nb, H=nb // cfg.blocks_per_req)
+    return cfg
+
+
+def cfg1_four_arms(device):
+    """config 1 under retrieval order, greedy, brute force over l(O,T) (trie-predicted) and brute force
+    over real hits (the exhaustive arm) — PAPER.md:195 does not say which objective its oracle ordering used."""
+    import torch
+    from itertools import permutations
+    from paper_2606_19667_b200.engine import TraceRunner
+    trace = tracegen.make_trace(tracegen.CONFIGS[1])
+    cfg = trace.cfg
+    out = {}
+    for arm in ("retrieval", "greedy", "brute_force_l", "exhaustive"):
+        run = TraceRunner(trace, "greedy" if arm == "brute_force_l" else arm, device=device)
+        if arm == "brute_force_l":          # the library predicts, the harness enumerates: first maximiser of cw_predict
+            def admit(r, run=run):
+                D = trace.retrieval[r]
+                best, best_l = list(D), -1
+                for p in permutations(range(len(D))):
+                    O = [D[i] for i in p]
+                    l = run.ctx.cw_predict(O)
+                    if list(p[l:]) == sorted(p[l:]) and l > best_l:
+                        best, best_l = O, l
+                tokens = tracegen.assemble_prompt(trace, r, best)
+                req, table, c = run.ctx.cw_lookup(tokens)
+                run.ctx.cw_observe(best)
+                from paper_2606_19667_b200.engine import RequestRecord
+                return req, RequestRecord(r, best, best_l, tokens, table, c, len(run.waves))
+            run._admit = admit
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        recs = run.run(keep_outputs=False)
+        e1.record()
+        torch.cuda.synchronize()
+        out[arm] = {"orders": [rec.order for rec in recs], "predicted_docs": [rec.depth for rec in recs],
+                    "hit_blocks": sum(rec.n_cached // 16 for rec in recs),
+                    "suffix_tokens": sum(cfg.n - rec.n_cached for rec in recs),
+                    "attn_flops": sum(4 * cfg.Hq * cfg.D * (cfg.n * (cfg.n + 1) // 2 - rec.n_cached * (rec.n_cached + 1) // 2) for rec in recs),
+                    "trace_ms_python_driven": e0.elapsed_time(e1)}
+    return out
 
 
 def run_sweep(args):
@@ -528,7 +617,14 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 4, 5])
+    ap.add_argument("--config", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--k", type=int, default=5, help="--config 3: top-k of the sweep cell")
+    ap.add_argument("--overlap", type=int, default=60, help="--config 3: adjacent overlap in percent")
+    ap.add_argument("--arm", default="greedy", help="ordering arm of the timed workload (cacheweaver.h CW_ARM_*)")
+    ap.add_argument("--one-wave", action="store_true", help="pool large enough for the whole batch (cfg 4 variant of SURVEY.md 8(d))")
+    ap.add_argument("--real-waves", type=int, default=0, help="with --device-inputs: tracegen activations for the first N waves")
+    ap.add_argument("--seconds", type=float, default=0.0, help="run the timed region for about this long (sustained figure)")
+    ap.add_argument("--skip-per-request", action="store_true")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--oracle-requests", type=int, default=None, help="requests in the oracle's bounded sample")
     ap.add_argument("--e2e-steps", type=int, default=5)
@@ -539,7 +635,7 @@ def main():
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.oracle_requests is None:
-        args.oracle_requests = {1: 4, 2: 16 if args.impl == "ours" else 4, 4: 1, 5: 1}[args.config]
+        args.oracle_requests = {1: 4, 2: 16 if args.impl == "ours" else 4, 3: 4, 4: 1, 5: 1}[args.config]
     if args.arms:
         run_arms(args)
     elif args.sweep:

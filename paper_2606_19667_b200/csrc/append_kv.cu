@@ -9,6 +9,8 @@
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
 
+#include <algorithm>
+
 #include "cw_internal.h"
 
 namespace cw {
@@ -32,13 +34,13 @@ __device__ __forceinline__ uint32_t f2_to_bf2(float a, float b) {
     return *reinterpret_cast<uint32_t*>(&h);
 }
 
-// rotate one (lo, hi) chunk pair: cs = 8 x {cos, sin} fp32 for the 8 frequencies of this chunk
-__device__ __forceinline__ void rope_pair(uint4& lo, uint4& hi, const float4* __restrict__ cs) {
+// rotate one (lo, hi) chunk pair: cs = 8 x {cos, sin} fp32 for the 8 frequencies of this chunk (in registers)
+__device__ __forceinline__ void rope_pair(uint4& lo, uint4& hi, const float4 (&cs)[4]) {
     uint32_t* l = reinterpret_cast<uint32_t*>(&lo);
     uint32_t* h = reinterpret_cast<uint32_t*>(&hi);
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-        float4 t = __ldg(cs + j);                       // {cos0, sin0, cos1, sin1}
+        const float4 t = cs[j];                         // {cos0, sin0, cos1, sin1}
         float2 a = bf2_to_f2(l[j]), b = bf2_to_f2(h[j]);
         float x0 = a.x * t.x - b.x * t.y, y0 = b.x * t.x + a.x * t.y;
         float x1 = a.y * t.z - b.y * t.w, y1 = b.y * t.z + a.y * t.w;
@@ -81,33 +83,52 @@ __global__ void __launch_bounds__(THREADS) append_kv_kernel(
         const int blk = __ldg(tables + (size_t)r * max_blocks + (p >> 4));
         const int tib = p & 15;
         const int prow = p < max_position ? p : max_position - 1;
-        const float4* cs_row = reinterpret_cast<const float4*>(rope_table + (size_t)prow * D);
-        for (int u = threadIdx.x; u < units; u += THREADS) {
-            if (u < uq) {
-                const int h = u / CPH, c = u % CPH;
-                const size_t off = ((size_t)tok * Hq + h) * D + c * 8;
-                uint4 a = ld_stream(q + off), b = ld_stream(q + off + D / 2);
-                rope_pair(a, b, cs_row + c * 4);
-                const int kvh = h / g, row = tloc * g + (h - kvh * g);
-                __nv_bfloat16* qb = q_roped + q_tile_base + (size_t)kvh * s_len * g * D + row * 64;
-                const int d0 = c * 8, d1 = c * 8 + D / 2;
-                st_stream(qb + (d0 >> 6) * rows_valid * 64 + ((((d0 & 63) >> 3) ^ (row & 7)) << 3), a);
-                st_stream(qb + (d1 >> 6) * rows_valid * 64 + ((((d1 & 63) >> 3) ^ (row & 7)) << 3), b);
-            } else if (u < uq + uk) {
-                const int uu = u - uq, h = uu / CPH, c = uu % CPH;
-                const size_t off = ((size_t)tok * Hkv + h) * D + c * 8;
-                uint4 a = ld_stream(k + off), b = ld_stream(k + off + D / 2);
-                rope_pair(a, b, cs_row + c * 4);
-                __nv_bfloat16* base = k_pool + ((size_t)blk * Hkv + h) * (16 * D);
-                st_stream(base + pool_chunk_offset<D>(tib, c * 8), a);
-                st_stream(base + pool_chunk_offset<D>(tib, c * 8 + D / 2), b);
-            } else {
-                const int uu = u - uq - uk, h = uu / CPH, c = uu % CPH;
-                const size_t off = ((size_t)tok * Hkv + h) * D + c * 8;
-                uint4 a = ld_stream(v + off), b = ld_stream(v + off + D / 2);
-                __nv_bfloat16* base = v_pool + ((size_t)blk * Hkv + h) * (16 * D);
-                st_stream(base + pool_chunk_offset<D>(tib, c * 8), a);
-                st_stream(base + pool_chunk_offset<D>(tib, c * 8 + D / 2), b);
+        // A thread's units are THREADS apart and THREADS % CPH == 0, so all of them rotate the same 8 frequencies: the
+        // {cos, sin} pairs are loaded once per token and thread (they would otherwise double the L1 load traffic).
+        static_assert(THREADS % CPH == 0, "chunk index must be the same for every unit of a thread");
+        float4 cs[4];
+        {
+            const float4* cs_row = reinterpret_cast<const float4*>(rope_table + (size_t)prow * D) + (threadIdx.x % CPH) * 4;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) cs[j] = __ldg(cs_row + j);
+        }
+        // Units are processed in groups of kUnroll per thread: all loads of a group are issued before the first store, so a
+        // thread keeps 2 * kUnroll 16-byte loads in flight (the kernel is bound by bytes in flight, not by arithmetic).
+        constexpr int kUnroll = 3;
+        for (int u0 = threadIdx.x; u0 < units; u0 += kUnroll * THREADS) {
+            uint4 lo[kUnroll], hi[kUnroll];
+#pragma unroll
+            for (int i = 0; i < kUnroll; ++i) {
+                const int u = u0 + i * THREADS;
+                if (u < units) {
+                    const __nv_bfloat16* src;
+                    if (u < uq) src = q + ((size_t)tok * Hq + u / CPH) * D + (u % CPH) * 8;
+                    else if (u < uq + uk) src = k + ((size_t)tok * Hkv + (u - uq) / CPH) * D + ((u - uq) % CPH) * 8;
+                    else src = v + ((size_t)tok * Hkv + (u - uq - uk) / CPH) * D + ((u - uq - uk) % CPH) * 8;
+                    lo[i] = ld_stream(src);
+                    hi[i] = ld_stream(src + D / 2);
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < kUnroll; ++i) {
+                const int u = u0 + i * THREADS;
+                if (u >= units) break;
+                if (u < uq) {
+                    const int h = u / CPH, c = u % CPH;
+                    rope_pair(lo[i], hi[i], cs);
+                    const int kvh = h / g, row = tloc * g + (h - kvh * g);
+                    __nv_bfloat16* qb = q_roped + q_tile_base + (size_t)kvh * s_len * g * D + row * 64;
+                    const int d0 = c * 8, d1 = c * 8 + D / 2;
+                    st_stream(qb + (d0 >> 6) * rows_valid * 64 + ((((d0 & 63) >> 3) ^ (row & 7)) << 3), lo[i]);
+                    st_stream(qb + (d1 >> 6) * rows_valid * 64 + ((((d1 & 63) >> 3) ^ (row & 7)) << 3), hi[i]);
+                } else {
+                    const bool is_k = u < uq + uk;
+                    const int uu = is_k ? u - uq : u - uq - uk, h = uu / CPH, c = uu % CPH;
+                    if (is_k) rope_pair(lo[i], hi[i], cs);
+                    __nv_bfloat16* base = (is_k ? k_pool : v_pool) + ((size_t)blk * Hkv + h) * (16 * D);
+                    st_stream(base + pool_chunk_offset<D>(tib, c * 8), lo[i]);
+                    st_stream(base + pool_chunk_offset<D>(tib, c * 8 + D / 2), hi[i]);
+                }
             }
         }
     }
@@ -121,23 +142,29 @@ int launch_append_kv(const cw_config& cfg, const void* q, const void* k, const v
     // threads per CTA: the multiple of 32 (<= 128) that leaves the fewest idle lanes in the last round over the token's
     // units (8B: 384 units = 3 x 128; 70B: 640 = 5 x 128; Qwen2.5-7B: 288 = 3 x 96) — idle lanes are bytes not in flight
     const int units = (cfg.num_q_heads + 2 * cfg.num_kv_heads) * (cfg.head_dim / 16);
+    int64_t grid = 0;
     int threads = 128, best_waste = 1 << 30;
     for (int t = 128; t >= 64; t -= 32) {
         const int waste = (units + t - 1) / t * t - units;
         if (waste < best_waste) { best_waste = waste; threads = t; }
     }
-    const int per_sm = 2048 / threads;
-    const int grid = T < num_sms * per_sm ? T : num_sms * per_sm;
+    // grid = one full wave of resident CTAs (occupancy is set by registers, asked from the runtime once per variant):
+    // a larger grid-stride grid would run a partial second wave
 #define CW_LAUNCH_APPEND(DD, TT)                                                                                \
-    append_kv_kernel<DD, TT><<<grid, TT, 0, s>>>(                                                               \
+    static int occ_##DD##_##TT = 0;                                                                             \
+    if (occ_##DD##_##TT == 0 &&                                                                                 \
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ_##DD##_##TT, append_kv_kernel<DD, TT>, TT, 0) != cudaSuccess) \
+        occ_##DD##_##TT = 2048 / TT;                                                                            \
+    grid = std::min<int64_t>(T, (int64_t)num_sms * std::max(1, occ_##DD##_##TT));                               \
+    append_kv_kernel<DD, TT><<<(unsigned)grid, TT, 0, s>>>(                                                               \
         (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, (__nv_bfloat16*)q_roped,     \
         (__nv_bfloat16*)cfg.k_pool, (__nv_bfloat16*)cfg.v_pool, (const float*)cfg.rope_table, cu, ncached,      \
         tables, max_blocks, B, T, cfg.num_q_heads, cfg.num_kv_heads, cfg.max_position)
 #define CW_LAUNCH_APPEND_D(DD)                                                                                  \
     do {                                                                                                        \
-        if (threads == 128) CW_LAUNCH_APPEND(DD, 128);                                                          \
-        else if (threads == 96) CW_LAUNCH_APPEND(DD, 96);                                                       \
-        else CW_LAUNCH_APPEND(DD, 64);                                                                          \
+        if (threads == 128) { CW_LAUNCH_APPEND(DD, 128); }                                                      \
+        else if (threads == 96) { CW_LAUNCH_APPEND(DD, 96); }                                                   \
+        else { CW_LAUNCH_APPEND(DD, 64); }                                                                      \
     } while (0)
     if (cfg.head_dim == 128) CW_LAUNCH_APPEND_D(128); else CW_LAUNCH_APPEND_D(64);
 #undef CW_LAUNCH_APPEND_D
