@@ -16,7 +16,8 @@ The hash chain is computed separately so the chain values can be compared bit-ex
 Readings where the paper is silent: FNV-1a-64 over parent(8 LE bytes) ‖ 16 tokens
 (4 LE bytes each); LRU free list, pop head, release in reverse block order to the tail; eager registration.
 Pins: tests/test_oracle_blocks.py (FNV-1a textbook vectors, hand-worked chain values, prefix sensitivity,
-the hand-worked block-table scenario of SURVEY.md §8(c7), invariants under random op sequences).
+the hand-worked block-table scenario of SURVEY.md §8(c7), invariants under random op sequences); extend():
+tests/test_oracle_extend.py (hand-worked tables, growth == one-shot lookup in tables and registrations, invariants).
 """
 from __future__ import annotations
 
@@ -64,6 +65,7 @@ class BlockManager:
         self.index = {}                            # prefix bytes -> block id
         self.free = OrderedDict((b, None) for b in range(num_blocks))   # head = first key
         self.reqs = {}
+        self.tokens_of = {}                        # request -> its token sequence so far (extend() appends to it)
         self.next_req = 1
         self.evictions = 0
         self.hit_blocks = 0
@@ -121,6 +123,7 @@ class BlockManager:
         req = self.next_req
         self.next_req += 1
         self.reqs[req] = (table, keys, m, nfull)
+        self.tokens_of[req] = np.ascontiguousarray(tokens, dtype="<i4").copy()
         if self.eager:
             self._register(table, keys, m, nfull)                                  # (5)
         self.hit_blocks += m
@@ -133,7 +136,38 @@ class BlockManager:
                 self.index[keys[i]] = table[i]
                 self.key_of[table[i]] = keys[i]
 
+    def extend(self, req, new_tokens):
+        """NEXT-4 (PAPER.md:253-283 continuous batching / decode): the live request grows by new_tokens
+        (a chunk of a chunked prefill, or generated tokens).  Blocks for the longer sequence are popped from the LRU head
+        exactly like in lookup step (4) (NoSpace leaves everything unchanged); with eager registration every block the new
+        tokens COMPLETE is registered under its whole token prefix (step (5)) — the formerly partial last block included.
+        Returns the request's block table."""
+        table, keys, m, nfull = self.reqs[req]
+        tokens = np.concatenate([self.tokens_of[req], np.ascontiguousarray(new_tokens, dtype="<i4")])
+        n = len(tokens)
+        need = -(-n // BS) - len(table)
+        if need > len(self.free):
+            raise NoSpace()
+        table = list(table)
+        for _ in range(need):
+            b, _ = self.free.popitem(last=False)
+            if self.key_of[b] is not None:
+                del self.index[self.key_of[b]]
+                self.key_of[b] = None
+                self.evictions += 1
+            self.ref[b] = 1
+            table.append(b)
+        new_nfull = n // BS
+        keys = self._prefix_keys(tokens, new_nfull)
+        self.reqs[req] = (table, keys, m, new_nfull)
+        self.tokens_of[req] = tokens
+        if self.eager:
+            self._register(table, keys, nfull, new_nfull)
+        self.miss_blocks += need
+        return table
+
     def release(self, req):
+        self.tokens_of.pop(req, None)
         table, keys, m, nfull = self.reqs.pop(req)
         if not self.eager:
             self._register(table, keys, m, nfull)

@@ -40,7 +40,7 @@ namespace {
 constexpr int kTileM = 128;          // MMA M (TMEM lanes); a Q tile uses the first tpt*g of them
 constexpr int kChunk = 64;           // keys per KV chunk (4 pool blocks)
 constexpr int kThreads = 512;
-constexpr int kRegsSoftmax = 144, kRegsOther = 112;   // 256 threads each: 256 * (144 + 112) = 65536 registers
+constexpr int kRegsSoftmax = 136, kRegsOther = 120;   // 256 threads each: 256 * (136 + 120) = 65536 registers
 constexpr int kWorkInts = 8;         // ints per work item
 constexpr float kRescaleThreshold = 8.0f;   // log2 units
 constexpr float kSpecLimit = 65536.f;       // bound on a row sum taken against a stale reference maximum
