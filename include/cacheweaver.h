@@ -151,6 +151,15 @@ int cw_lookup(cw_ctx* ctx, const int32_t* tokens, int32_t n, int32_t peek_only,
               int64_t* out_req, int32_t* out_block_table, int32_t* out_n_cached);
 /* Unpin; blocks whose refcount reaches 0 go to the LRU tail in REVERSE block order. */
 int cw_release(cw_ctx* ctx, int64_t req);
+/* NEXT-4 (PAPER.md:253-283 continuous batching): the live request `req` grows by new_tokens[n_new]
+ * (host) — the next chunk of a chunked prefill, or generated tokens.  Blocks for the longer sequence are popped from the
+ * LRU head as in cw_lookup (CW_ERR_NO_SPACE leaves everything unchanged); with eager registration every block the new
+ * tokens complete is hashed, chained to the request's last full block, and entered into the prefix index (the formerly
+ * partial last block included).  out_block_table[cap] (host) receives the whole table, *out_n_blocks its length.
+ * The K/V of the new tokens are written by the next cw_append_kv / cw_prefill_requests of this request, whose n_cached
+ * is the number of tokens already in the pool (no longer a multiple of 16). */
+int cw_extend(cw_ctx* ctx, int64_t req, const int32_t* new_tokens, int32_t n_new, int32_t* out_block_table, int32_t cap,
+              int32_t* out_n_blocks);
 /* Back to the state right after cw_create: empty knowledge tree, empty prefix index, LRU list 0..NB-1, no live
  * requests, statistics zeroed.  Pools and the RoPE table are untouched (old KV is unreachable: nothing is indexed). */
 int cw_reset(cw_ctx* ctx);
@@ -180,7 +189,9 @@ int cw_free_list(cw_ctx* ctx, int32_t* out, int32_t cap, int32_t* out_len);
 
 /* ---- device work (async on `stream`) ----------------------------------------------------------------- */
 /* Batch of B requests; request r owns suffix rows cu_seqlens_q[r]..cu_seqlens_q[r+1]-1 (T rows in total),
- * row i of request r sits at absolute prompt position n_cached[r] + i.  All d_* pointers are DEVICE int32.
+ * row i of request r sits at absolute prompt position n_cached[r] + i; n_cached[r] = tokens of the request already in
+ * the pool (16 * matched blocks after cw_lookup; any value for a later chunk of a chunked prefill or a decode row,
+ * SURVEY.md 8(f) NEXT-4).  All d_* pointers are DEVICE int32.
  * d_block_tables is [B, max_blocks_per_req] row-major.
  *
  * cw_append_kv — fused RoPE + KV scatter (kernel 1):  for each suffix token at position p
@@ -204,8 +215,8 @@ int cw_append_kv(cw_ctx* ctx, const void* q, const void* k, const void* v, void*
  *   max_q_len / max_kv_len: upper bounds on the suffix length / kv length of any request of the batch (host values;
  *   max_kv_len <= 16 * max_blocks_per_req and <= max_position).
  *   d_work: DEVICE int32 scratch of cw_attn_work_ints(ctx, B, T) ints, caller-owned, written by this call.  After the
- *   stream has run the call: d_work[1] != 0 means a request descriptor was invalid (n_cached not a multiple of 16,
- *   lengths beyond the stated maxima, kv_len mismatch) and that request produced no output; d_work[2] counts the
+ *   stream has run the call: d_work[1] != 0 means a request descriptor was invalid (negative lengths, lengths beyond
+ *   the stated maxima, kv_len mismatch) and that request produced no output; d_work[2] counts the
  *   softmax chunks that left the speculative path (statistics); d_work[3] is the number of work items.
  *   q_roped: as written by cw_append_kv (tile-packed); out [T,Hq,D] device bf16 row-major.
  *   (SURVEY.md 8(b) lists this signature without d_work; the scratch is passed in because the library allocates no
@@ -218,7 +229,8 @@ int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out,
 
 /* cw_prefill_requests — steps a7 + a8 for a wave of admitted requests in ONE call: the descriptors (cu_seqlens_q,
  * n_cached, block tables) are taken from the request handles reqs[0..B-1] (HOST, as returned by cw_lookup /
- * cw_admit_batch, in batch order), written to a library-owned pinned staging slot, copied to d_ws with one
+ * cw_admit_batch, in batch order; a request's rows are its tokens not yet written to the pool: the uncached suffix after
+ * cw_lookup, the appended tokens after cw_extend — prefill suffixes, prefill chunks and decode rows can share a call), written to a library-owned pinned staging slot, copied to d_ws with one
  * asynchronous H2D copy, and cw_append_kv + cw_prefill_attn are enqueued on `stream`.  Nothing is synchronised.
  *   q [T,Hq,D], k, v [T,Hkv,D], q_roped, out: device bf16 as in cw_append_kv / cw_prefill_attn; T must equal the sum
  *   of the requests' suffix lengths.  max_blocks_per_req >= the largest block-table length of the wave.

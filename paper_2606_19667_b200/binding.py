@@ -78,6 +78,7 @@ def load_library(build_if_missing: bool = True):
         "cw_hash_chain": (C.c_int, [vp, p(i32), i32, p(C.c_uint64)]),
         "cw_lookup": (C.c_int, [vp, p(i32), i32, i32, p(i64), p(i32), p(i32)]),
         "cw_release": (C.c_int, [vp, i64]),
+        "cw_extend": (C.c_int, [vp, i64, p(i32), i32, p(i32), i32, p(i32)]),
         "cw_free_list": (C.c_int, [vp, p(i32), i32, p(i32)]),
         "cw_reset": (C.c_int, [vp]),
         "cw_admit_batch": (C.c_int, [vp, p(i64), i32, i32, i32, p(i32), i32, i32, p(i32), i32, p(i64), p(i32), p(i64),
@@ -101,7 +102,7 @@ def load_library(build_if_missing: bool = True):
 
 
 EXPORTS = ["cw_create", "cw_destroy", "cw_strerror", "cw_last_error", "cw_stats", "cw_pool_bytes", "cw_pool_offset", "cw_q_roped_offset",
-           "cw_order", "cw_predict", "cw_order_arm", "cw_observe", "cw_mark_stale", "cw_feedback", "cw_hash_chain", "cw_lookup", "cw_release", "cw_free_list",
+           "cw_order", "cw_predict", "cw_order_arm", "cw_observe", "cw_mark_stale", "cw_feedback", "cw_hash_chain", "cw_lookup", "cw_release", "cw_extend", "cw_free_list",
            "cw_reset", "cw_admit_batch", "cw_release_batch",
            "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_prefill_requests_ws_bytes",
            "cw_prefill_requests_work_offset", "cw_prefill_requests", "cw_gather_kv", "cw_prefill_host_ws_bytes",
@@ -232,6 +233,15 @@ class Context:
 
     def cw_release(self, req):
         self._check(self.lib.cw_release(self.h, req))
+
+    def cw_extend(self, req, new_tokens, cap=None):
+        """the live request grows by new_tokens; returns its whole block table (numpy int32)."""
+        t = _np_i32(new_tokens)
+        cap = int(cap) if cap is not None else self.NB
+        table = np.empty(cap, dtype=np.int32)
+        nb = C.c_int32()
+        self._check(self.lib.cw_extend(self.h, req, _i32p(t), len(t), _i32p(table), cap, C.byref(nb)))
+        return table[: nb.value].copy()
 
     def cw_reset(self):
         self._check(self.lib.cw_reset(self.h))

@@ -273,6 +273,15 @@ int cw_release(cw_ctx* ctx, int64_t req) {
     return ctx->blocks->release(req);
 }
 
+int cw_extend(cw_ctx* ctx, int64_t req, const int32_t* new_tokens, int32_t n_new, int32_t* out_block_table, int32_t cap,
+              int32_t* out_n_blocks) {
+    if (!ctx || n_new < 0 || (n_new > 0 && !new_tokens) || !out_block_table || !out_n_blocks || cap < 0)
+        return fail(ctx, CW_ERR_INVALID, "cw_extend: bad argument");
+    int rc = ctx->blocks->extend(req, new_tokens, n_new, out_block_table, cap, out_n_blocks);
+    if (rc == CW_ERR_INVALID) return fail(ctx, rc, "cw_extend: block table capacity too small (or sequence too long)");
+    return rc;
+}
+
 int cw_reset(cw_ctx* ctx) {
     if (!ctx) return CW_ERR_INVALID;
     delete ctx->tree;
@@ -466,7 +475,7 @@ int cw_prefill_requests(cw_ctx* ctx, const int64_t* reqs, int32_t B, const void*
     for (int32_t r = 0; r < B; ++r) {
         const cw::Request* rq = ctx->blocks->find(reqs[r]);
         if (!rq) return fail(ctx, CW_ERR_BAD_HANDLE, "cw_prefill_requests: unknown request handle");
-        const int32_t nblk = (int32_t)rq->table.size(), c = rq->m * CW_BLOCK_SIZE, s = rq->n - c;
+        const int32_t nblk = (int32_t)rq->table.size(), c = rq->n_done, s = rq->n - c;
         if (nblk > max_blocks) return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: max_blocks too small for a request");
         if (rq->n > ctx->cfg.max_position) return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: prompt longer than max_position");
         nc[r] = c;
@@ -476,7 +485,11 @@ int cw_prefill_requests(cw_ctx* ctx, const int64_t* reqs, int32_t B, const void*
         max_q = std::max(max_q, s);
         max_kv = std::max(max_kv, rq->n);
     }
-    if (cu[B] != T) return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: T does not match the requests' suffix lengths");
+    if (cu[B] != T) return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: T does not match the requests' pending tokens");
+    for (int32_t r = 0; r < B; ++r) {          // everything up to n is now (being) written: the next call starts there
+        cw::Request* rq = ctx->blocks->find_mut(reqs[r]);
+        rq->n_done = rq->n;
+    }
     auto s = static_cast<cudaStream_t>(stream);
     char* ws = static_cast<char*>(d_ws);
     e = cudaMemcpyAsync(ws, st.host, desc_bytes, cudaMemcpyHostToDevice, s);
@@ -533,8 +546,8 @@ int cw_prefill_host(cw_ctx* ctx, const void* h_q, const void* h_k, const void* h
     int32_t max_q = 0, max_kv = 0;
     for (int r = 0; r < B; ++r) {
         const int s = h_cu[r + 1] - h_cu[r];
-        if (s < 0 || h_nc[r] < 0 || h_nc[r] % CW_BLOCK_SIZE != 0 ||
-            (int64_t)h_nc[r] + s > (int64_t)max_blocks * CW_BLOCK_SIZE || h_nc[r] + s > ctx->cfg.max_position)
+        if (s < 0 || h_nc[r] < 0 || (int64_t)h_nc[r] + s > (int64_t)max_blocks * CW_BLOCK_SIZE ||
+            h_nc[r] + s > ctx->cfg.max_position)
             return fail(ctx, CW_ERR_INVALID, "cw_prefill_host: bad request descriptor");
         max_q = std::max(max_q, s);
         max_kv = std::max(max_kv, h_nc[r] + s);

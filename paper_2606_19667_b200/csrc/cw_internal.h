@@ -70,7 +70,9 @@ struct Request {
     std::vector<int32_t> table;
     std::vector<uint64_t> chain;
     int32_t m;      // matched (cached) blocks
-    int32_t n;      // prompt length in tokens
+    int32_t n;      // sequence length in tokens (prompt + what cw_extend appended)
+    int32_t n_done; // tokens whose K/V are (being) written to the pool: m*16 at lookup, advanced by cw_prefill_requests
+    int32_t tail[CW_BLOCK_SIZE];   // tokens of the trailing partial block (n % 16 of them): cw_extend completes it
 };
 
 class BlockManager {
@@ -91,6 +93,12 @@ class BlockManager {
     // returns CW_OK / CW_ERR_NO_SPACE
     int lookup(const int32_t* tokens, int32_t n, int64_t* req, int32_t* table, int32_t* n_cached);
     int release(int64_t req);
+    // NEXT-4: the live request grows by n_new tokens (chunked prefill / generated tokens).  CW_ERR_NO_SPACE: unchanged.
+    int extend(int64_t req, const int32_t* tokens, int32_t n_new, int32_t* table_out, int32_t cap, int32_t* n_blocks);
+    Request* find_mut(int64_t req) {
+        auto it = reqs_.find(req);
+        return it == reqs_.end() ? nullptr : &it->second;
+    }
     const Request* find(int64_t req) const {
         auto it = reqs_.find(req);
         return it == reqs_.end() ? nullptr : &it->second;

@@ -4,6 +4,7 @@
 #include "cw_internal.h"
 
 #include <algorithm>
+#include <climits>
 #include <cstring>
 
 namespace cw {
@@ -176,7 +177,9 @@ int BlockManager::lookup(const int32_t* tokens, int32_t n, int64_t* req, int32_t
     chain(tokens, n, r.chain);
     int32_t nblk = (n + CW_BLOCK_SIZE - 1) / CW_BLOCK_SIZE, nfull = n / CW_BLOCK_SIZE;
     r.n = n;
+    std::memcpy(r.tail, tokens + (size_t)nfull * CW_BLOCK_SIZE, sizeof(int32_t) * (size_t)(n - nfull * CW_BLOCK_SIZE));
     r.m = match(r.chain, n);                                                    // (1)
+    r.n_done = r.m * CW_BLOCK_SIZE;
     r.table.resize((size_t)nblk);
     int32_t matched_free = 0;
     for (int32_t i = 0; i < r.m; ++i) {
@@ -210,11 +213,59 @@ int BlockManager::lookup(const int32_t* tokens, int32_t n, int64_t* req, int32_t
     return CW_OK;
 }
 
+// NEXT-4: blocks for the longer sequence are popped from the LRU head like in lookup step (4); every
+// block the new tokens complete is hashed (chained to the request's last full block) and, with eager registration,
+// entered into the index (step (5)) — the formerly partial last block included.
+int BlockManager::extend(int64_t req, const int32_t* tokens, int32_t n_new, int32_t* table_out, int32_t cap, int32_t* n_blocks) {
+    auto it = reqs_.find(req);
+    if (it == reqs_.end()) return CW_ERR_BAD_HANDLE;
+    Request& r = it->second;
+    const int64_t n_total = (int64_t)r.n + n_new;
+    if (n_total > INT32_MAX) return CW_ERR_INVALID;
+    const int32_t nblk = (int32_t)((n_total + CW_BLOCK_SIZE - 1) / CW_BLOCK_SIZE);
+    const int32_t need = nblk - (int32_t)r.table.size();
+    if (nblk > cap) return CW_ERR_INVALID;
+    if (need > free_count_) return CW_ERR_NO_SPACE;
+    for (int32_t i = 0; i < need; ++i) {
+        int32_t b = next_[NB_];
+        unlink(b);
+        if (has_hash_[(size_t)b]) {
+            index_.erase(hash_[(size_t)b]);
+            has_hash_[(size_t)b] = 0;
+            ++evictions;
+        }
+        ref_[(size_t)b] = 1;
+        r.table.push_back(b);
+    }
+    const int32_t old_full = (int32_t)r.chain.size();
+    int32_t n_tail = r.n - old_full * CW_BLOCK_SIZE;
+    uint64_t parent = old_full ? r.chain.back() : salt_;
+    for (int32_t i = 0; i < n_new; ++i) {
+        r.tail[n_tail++] = tokens[i];
+        if (n_tail == CW_BLOCK_SIZE) {
+            parent = block_hash(parent, r.tail);
+            r.chain.push_back(parent);
+            n_tail = 0;
+        }
+    }
+    r.n = (int32_t)n_total;
+    if (eager_) {
+        const int32_t m_keep = r.m;
+        r.m = old_full;                       // reg() registers blocks [m, nfull): only the newly completed ones
+        reg(r, (int32_t)r.chain.size());
+        r.m = m_keep;
+    }
+    miss_blocks += need;
+    std::memcpy(table_out, r.table.data(), sizeof(int32_t) * r.table.size());
+    *n_blocks = nblk;
+    return CW_OK;
+}
+
 int BlockManager::release(int64_t req) {
     auto it = reqs_.find(req);
     if (it == reqs_.end()) return CW_ERR_BAD_HANDLE;
     Request& r = it->second;
-    if (!eager_) reg(r, (int32_t)r.chain.size());
+    if (!eager_) reg(r, (int32_t)r.chain.size());     // lazy registration: everything the request completed, at release
     for (int32_t i = (int32_t)r.table.size() - 1; i >= 0; --i) {               // reverse: deepest evicted first
         int32_t b = r.table[(size_t)i];
         if (--ref_[(size_t)b] == 0) push_tail(b);

@@ -592,6 +592,8 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
 // so the tail of the launch is made of short items); inside a request kv-head major, tile pairs by descending kv length.
 // CTA b takes items b, b+G, b+2G, ...: the CTAs work on neighbouring items of the same (request, kv head) at the same
 // time and share its K/V blocks through L2.
+// n_cached[r] is the number of tokens of request r already in the pool: a multiple of 16 after cw_lookup, any value for a
+// chunk of a chunked prefill or a decode row.
 // work header (ints): [0] claim counter, [1] error flags (bit 0: a request descriptor was invalid and contributes no
 // item), [2] exact-path fallbacks of the speculative softmax (statistics), [3] number of items; items from int 8 on.
 constexpr int kSchedMaxSmemReqs = 2048;      // requests whose (suffix, cached, offset) fit the schedule kernel's shared memory
@@ -614,7 +616,7 @@ __global__ void __launch_bounds__(1024) attn_schedule_kernel(
         const int lo = cu[r], hi = cu[r + 1];
         c = nc[r];
         const int64_t s = (int64_t)hi - lo;
-        const bool ok = lo >= 0 && s >= 0 && hi <= T && c >= 0 && c % CW_BLOCK_SIZE == 0 && s <= max_q_len &&
+        const bool ok = lo >= 0 && s >= 0 && hi <= T && c >= 0 && s <= max_q_len &&
                         (int64_t)c + s <= max_kv_len && (int64_t)c + s <= (int64_t)max_blocks * CW_BLOCK_SIZE &&
                         (int64_t)c + s <= max_position && (kv_len == nullptr || kv_len[r] == c + s);
         return ok ? (int)s : -1;

@@ -219,10 +219,10 @@ def test_empty_batch_and_bad_descriptors(dev):
     q = torch.zeros(20, 2, 64, dtype=torch.bfloat16, device=dev)
     with pytest.raises(CwError):                                               # max_kv_len beyond the block table
         b.ctx.cw_prefill_attn(q, torch.empty_like(q), z, z, b.d_tables, b.max_blocks, 1, 20, 20, 16 * b.max_blocks + 1, z)
-    # descriptors live on the device: an invalid one (n_cached not a multiple of 16) is rejected there — the request
+    # descriptors live on the device: an invalid one (here n_cached + s beyond max_kv_len) is rejected there — the request
     # produces no output and the error flag of the work header is set
     d_cu = torch.tensor([0, 20], dtype=torch.int32, device=dev)
-    d_nc = torch.tensor([8], dtype=torch.int32, device=dev)
+    d_nc = torch.tensor([16], dtype=torch.int32, device=dev)
     work = torch.zeros(b.ctx.cw_attn_work_ints(1, 20), dtype=torch.int32, device=dev)
     out = torch.full_like(q, float("nan"))
     b.ctx.cw_prefill_attn(q, out, d_cu, d_nc, b.d_tables, b.max_blocks, 1, 20, 20, 20, work)
@@ -385,6 +385,80 @@ def test_prefill_attn_returns_before_the_stream_reaches_it(dev):
     torch.cuda.synchronize()
     assert int(work[1]) == 0 and int(work[3]) == B * Hkv * (s // (2 * (128 // (Hq // Hkv))))
     assert np.median(host_us[1:]) < 60.0, host_us               # ctypes marshalling + two launches
+
+
+def test_mixed_batch_prefill_chunks_and_decode_rows(dev):
+    """NEXT-4: one varlen launch holding a cold prefill, a prefix-cached suffix, the
+    second chunk of a chunked prefill (133 tokens already in the pool — not a multiple of 16) and single-token decode rows
+    over long contexts.  Every row against the fp64 oracle's full recompute."""
+    cs = [0, 256, 133, 1000, 37, 1327, 640]
+    ss = [200, 48, 100, 1, 1, 1, 1]
+    b = Batch(dev, 32, 8, 128, cs, ss, seed=31)
+    _, out_bits, cu = b.run()
+    for r in range(b.B):
+        assert_close_attn(out_bits[cu[r]:cu[r + 1]], b.oracle(r), f"r={r} past={cs[r]} rows={ss[r]}")
+
+
+def test_chunked_prefill_and_decode_through_request_handles(dev):
+    """cw_lookup, then the prompt's uncached suffix in one cw_prefill_requests call; then cw_extend + cw_prefill_requests
+    for two more chunks (37 and 64 tokens) and four decode steps of one token each, sharing launches with a second
+    request that is being prefilled.  Outputs equal the oracle's full recompute of the final sequences; block tables equal
+    the oracle block manager's."""
+    from oracle.blocks import BlockManager
+    rng = np.random.default_rng(41)
+    Hq, Hkv, D, theta, NB = 8, 2, 128, 5e5, 64
+    ctx = Context(NB, Hq, Hkv, D, 4, rope_theta=theta, max_position=512, device=dev)
+    obm = BlockManager(NB)
+    n_final = [100 + 37 + 64 + 4, 150]
+    toks = [rng.integers(0, 32000, n, dtype=np.int32) for n in n_final]
+    q = [rand_bits(rng, n, Hq, D) for n in n_final]
+    k = [rand_bits(rng, n, Hkv, D) for n in n_final]
+    v = [rand_bits(rng, n, Hkv, D) for n in n_final]
+    outs = [np.zeros((n, Hq, D), dtype=np.uint16) for n in n_final]
+    reqs, oreqs, done = [None, None], [None, None], [0, 0]
+    max_blocks = 16
+
+    def launch(batch):                      # batch: list of (request index, tokens now in the sequence)
+        rows = [(r, done[r], upto) for r, upto in batch]
+        cat = lambda xs: to_dev(np.concatenate([xs[r][lo:hi] for r, lo, hi in rows], axis=0), dev)
+        dq, dk, dv = cat(q), cat(k), cat(v)
+        T = dq.shape[0]
+        qr, out = torch.empty_like(dq), torch.full_like(dq, float("nan"))
+        ws = torch.empty(ctx.cw_prefill_requests_ws_bytes(len(rows), T, max_blocks), dtype=torch.uint8, device=dev)
+        ctx.cw_prefill_requests([reqs[r] for r, _, _ in rows], dq, dk, dv, qr, out, T, max_blocks, ws)
+        torch.cuda.synchronize()
+        o, pos = to_bits(out), 0
+        for r, lo, hi in rows:
+            outs[r][lo:hi] = o[pos:pos + hi - lo]
+            pos += hi - lo
+            done[r] = hi
+
+    # step 1: request 0 admitted with its first 100 tokens
+    reqs[0], table, c = ctx.cw_lookup(toks[0][:100])
+    oreqs[0], otable, oc = obm.lookup(toks[0][:100])
+    assert (table.tolist(), c) == (otable, oc)
+    done[0] = c
+    launch([(0, 100)])
+    # step 2: request 0 grows by a 37-token chunk; request 1 is admitted (150 tokens) and prefilled in the same launch
+    assert ctx.cw_extend(reqs[0], toks[0][100:137]).tolist() == obm.extend(oreqs[0], toks[0][100:137])
+    reqs[1], table, c = ctx.cw_lookup(toks[1])
+    oreqs[1], otable, oc = obm.lookup(toks[1])
+    assert (table.tolist(), c) == (otable, oc)
+    done[1] = c
+    launch([(0, 137), (1, 150)])
+    # step 3: a 64-token chunk, then four decode steps
+    assert ctx.cw_extend(reqs[0], toks[0][137:201]).tolist() == obm.extend(oreqs[0], toks[0][137:201])
+    launch([(0, 201)])
+    for t in range(201, 205):
+        assert ctx.cw_extend(reqs[0], toks[0][t:t + 1]).tolist() == obm.extend(oreqs[0], toks[0][t:t + 1])
+        launch([(0, t + 1)])
+    assert ctx.cw_free_list() == obm.free_list()
+    f = tracegen.bf16_bits_to_f64
+    for r in range(2):
+        assert_close_attn(outs[r], oattn.attention_full(f(q[r]), f(k[r]), f(v[r]), theta), f"request {r}")
+    # a later request with the same 201 leading tokens hits every block the chunks completed
+    probe = np.concatenate([toks[0][:201], rng.integers(0, 32000, 9, dtype=np.int32)])
+    assert ctx.cw_lookup(probe, peek_only=True) == 16 * obm.match(probe) == 192
 
 
 def test_prefill_requests_equals_separate_calls(dev):

@@ -282,3 +282,47 @@ def test_admit_batch_invalid_row_leaves_state_untouched():
     assert (ctx.cw_stats(), ctx.cw_free_list()) == before
     a = ctx.cw_admit_batch(np.array([[0, 1, 2], [3, 1, 0]], dtype=np.int64), "greedy", doc_tokens, queries[:2])
     assert a["admitted"] == 2
+
+
+@pytest.mark.parametrize("seed", range(4))
+def test_extend_matches_oracle_under_random_growth(seed):
+    """cw_extend vs oracle BlockManager.extend: several live requests grow in random pieces (with shared prefixes and a pool
+    small enough for NO_SPACE), block tables / free lists / hit counts bit-exact, NO_SPACE leaves both sides unchanged."""
+    rng = np.random.default_rng(200 + seed)
+    NB = 40
+    ctx = Context(NB, 2, 1, 64, 4)
+    obm = BlockManager(NB)
+    base = rng.integers(0, 32000, 96, dtype=np.int32)
+    live = []
+    for step in range(120):
+        op = rng.integers(0, 10)
+        if op < 3 and len(live) < 5:
+            t = np.concatenate([base[: int(rng.integers(0, 97))], rng.integers(0, 32000, int(rng.integers(1, 40)), dtype=np.int32)])
+            try:
+                oreq, otable, oc = obm.lookup(t)
+            except OracleNoSpace:
+                with pytest.raises(NoSpace):
+                    ctx.cw_lookup(t)
+                continue
+            req, table, c = ctx.cw_lookup(t)
+            assert (table.tolist(), c) == (otable, oc)
+            live.append((req, oreq))
+        elif op < 8 and live:
+            req, oreq = live[int(rng.integers(0, len(live)))]
+            t = rng.integers(0, 32000, int(rng.integers(1, 30)), dtype=np.int32)
+            try:
+                otable = obm.extend(oreq, t)
+            except OracleNoSpace:
+                with pytest.raises(NoSpace):
+                    ctx.cw_extend(req, t)
+                assert ctx.cw_free_list() == obm.free_list()
+                continue
+            assert ctx.cw_extend(req, t).tolist() == otable
+        elif live:
+            req, oreq = live.pop(int(rng.integers(0, len(live))))
+            ctx.cw_release(req)
+            obm.release(oreq)
+        assert ctx.cw_free_list() == obm.free_list()
+        obm.check_invariants()
+    st = ctx.cw_stats()
+    assert (st["hit_blocks"], st["miss_blocks"], st["evictions"]) == (obm.hit_blocks, obm.miss_blocks, obm.evictions)
