@@ -572,6 +572,64 @@ def run_sweep(args):
     return cells
 
 
+def run_mixed(args):
+    """SURVEY.md 8(f) NEXT-4 (continuous batching): decode rows and prefill suffixes in the same varlen
+    launch, 8B shapes.  Three launches are timed: (a) 512 single-token decode rows over 1024..8192-token contexts — bound by
+    reading each context's K/V once (AI = g = 4 flop/B, far below the 263 flop/B ridge), reported against the HBM peak;
+    (b) 64 prefill suffixes of 1072 tokens behind a 256-token cached prefix; (c) both in one launch."""
+    import torch
+    from paper_2606_19667_b200 import Context
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback")
+    dev, pk = "cuda:0", peaks()
+    Hq, Hkv, D = 32, 8, 128
+    rng = np.random.default_rng(0)
+    dec_n = rng.integers(1024, 8193, size=512)                 # tokens already in the pool per decode row
+    pre_c, pre_s = np.full(64, 256), np.full(64, 1072)
+    def build(cs, ss):
+        ns = cs + ss
+        nblk = -(-ns // 16)
+        mb = int(nblk.max())
+        tables = np.zeros((len(cs), mb), dtype=np.int32)
+        o = 0
+        for r, nb in enumerate(nblk):
+            tables[r, :nb] = np.arange(o, o + nb)
+            o += nb
+        cu = np.zeros(len(cs) + 1, dtype=np.int32)
+        cu[1:] = np.cumsum(ss)
+        return dict(cs=cs, ss=ss, ns=ns, tables=tables, cu=cu, blocks=o, mb=mb)
+    cases = {"decode_rows": build(dec_n, np.ones(512, dtype=np.int64)), "prefill_suffixes": build(pre_c, pre_s),
+             "mixed": build(np.concatenate([pre_c, dec_n]), np.concatenate([pre_s, np.ones(512, dtype=np.int64)]))}
+    NB = max(c["blocks"] for c in cases.values()) + 8
+    ctx = Context(NB, Hq, Hkv, D, 4, rope_theta=5e5, max_position=int(max(c["ns"].max() for c in cases.values())), device=dev)
+    g = torch.Generator(device=dev)
+    g.manual_seed(0)
+    ctx.k_pool.normal_(generator=g)
+    ctx.v_pool.normal_(generator=g)
+    for name, c in cases.items():
+        B, T = len(c["cs"]), int(c["cu"][-1])
+        q = torch.randn(T, Hq, D, device=dev, dtype=torch.bfloat16, generator=g)
+        k = torch.randn(T, Hkv, D, device=dev, dtype=torch.bfloat16, generator=g)
+        v = torch.randn(T, Hkv, D, device=dev, dtype=torch.bfloat16, generator=g)
+        qr, out = torch.empty_like(q), torch.empty_like(q)
+        d_cu, d_nc = torch.from_numpy(c["cu"]).to(dev), torch.from_numpy(c["cs"].astype(np.int32)).to(dev)
+        d_t = torch.from_numpy(c["tables"]).to(dev)
+        work = torch.empty(ctx.cw_attn_work_ints(B, T), dtype=torch.int32, device=dev)
+        ctx.cw_append_kv(q, k, v, qr, d_cu, d_nc, d_t, c["mb"], B, T)
+        fn = lambda: ctx.cw_prefill_attn(qr, out, d_cu, d_nc, d_t, c["mb"], B, T, int(c["ss"].max()), int(c["ns"].max()), work)
+        for _ in range(max(3, args.warmup)):
+            fn()
+        ms = timed(torch, fn, args.steps, None) / args.steps
+        flops = int(sum(4 * Hq * D * (int(n) * (int(n) + 1) // 2 - int(cc) * (int(cc) + 1) // 2) for n, cc in zip(c["ns"], c["cs"])))
+        kv_bytes = int(sum(2 * int(n) * Hkv * D * 2 for n in c["ns"])) + 2 * T * Hq * D * 2      # K, V once + q in, o out
+        line = {"case": name, "requests": B, "rows": T, "ms": ms, "attn_tflops": flops / ms / 1e9,
+                "algorithmic_bytes": kv_bytes, "gbs": kv_bytes / ms / 1e6, "frac_of_hbm_peak": kv_bytes / ms / 1e6 / pk["hbm"],
+                "frac_of_bf16_peak": flops / ms / 1e9 / pk["bf16"], "flop_per_byte": flops / kv_bytes,
+                "bound": "hbm" if flops / kv_bytes < 263 else "tensor", "fallbacks": int(work[2])}
+        print(json.dumps(line), flush=True)
+        del q, k, v, qr, out
+
+
 def run_arms(args):
     """Ordering arms of the paper's Table 4 on the bench configuration: retrieval, sorted, recency,
     greedy (Algorithm 1), exhaustive.  One JSON line per arm with hit blocks, suffix tokens, attention flops, host admission
@@ -630,13 +688,16 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--skip-retrieval", action="store_true")
     ap.add_argument("--device-inputs", action="store_true", help="timing-only: draw q,k,v on the device (no e2e leg)")
+    ap.add_argument("--mixed", action="store_true", help="NEXT-4: decode rows / prefill suffixes / both in one varlen launch, one JSON line each")
     ap.add_argument("--arms", action="store_true", help="ordering arms of the paper's Table 4 on --config, one JSON line per arm")
     ap.add_argument("--sweep", action="store_true", help="overlap x top-k sweep (BASELINE.json configs[2]), one JSON line per cell")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.oracle_requests is None:
         args.oracle_requests = {1: 4, 2: 16 if args.impl == "ours" else 4, 3: 4, 4: 1, 5: 1}[args.config]
-    if args.arms:
+    if args.mixed:
+        run_mixed(args)
+    elif args.arms:
         run_arms(args)
     elif args.sweep:
         run_sweep(args)
