@@ -630,6 +630,53 @@ def run_mixed(args):
         del q, k, v, qr, out
 
 
+def run_layouts(args):
+    """config 2's trace under the paper-literal prompt layout (instruction + [Document r: id] headers,
+    180-220-token documents) against the block-aligned plain layout with the same retrieval lists:
+    hit blocks, suffix tokens, attention flops and prefill ms (one wave, both kernels) per layout and ordering arm."""
+    import dataclasses
+    import torch
+    from paper_2606_19667_b200.engine import TraceRunner
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback")
+    dev = "cuda:0"
+    base = tracegen.CONFIGS[2]
+    layouts = {"plain-aligned-208": dataclasses.replace(base, name="cfg2-plain208", doc_len=208, admission="waves"),
+               "literal-200+-20": dataclasses.replace(base, name="cfg2-literal", doc_len=200, doc_jitter=20, layout="literal",
+                                                      admission="waves")}
+    for lname, cfg in layouts.items():
+        cfg = dataclasses.replace(cfg, H=cfg.NB // (-(-cfg.n // 16)))
+        trace = tracegen.make_trace(cfg)
+        for arm in ("retrieval", "greedy", "greedy_feedback"):
+            run = TraceRunner(trace, arm, device=dev)
+            waves = []
+            run.prefill_wave = lambda wave, keep_outputs=True: waves.append(wave)      # host path only; the wave is timed below
+            recs = run.run(compute=True, keep_outputs=False)
+            assert len(waves) == 1
+            wave = waves[0]
+            ns = np.array([len(rec.tokens) for rec in recs])
+            nc = np.array([rec.n_cached for rec in recs])
+            flops = int(sum(4 * cfg.Hq * cfg.D * (int(n) * (int(n) + 1) // 2 - int(c) * (int(c) + 1) // 2) for n, c in zip(ns, nc)))
+            # the wave was released by run(); re-admit nothing: replay the recorded descriptors (both kernels are idempotent)
+            q, k, v = run.wave_inputs(wave)
+            d_cu, d_nc, d_t, work = run.wave_descriptors(wave)
+            qr, out = torch.empty_like(q), torch.empty_like(q)
+            s = np.diff(wave.cu)
+            def fn():
+                run.ctx.cw_append_kv(q, k, v, qr, d_cu, d_nc, d_t, wave.max_blocks, wave.B, wave.T)
+                run.ctx.cw_prefill_attn(qr, out, d_cu, d_nc, d_t, wave.max_blocks, wave.B, wave.T, int(s.max()),
+                                        int((wave.nc + s).max()), work)
+            for _ in range(max(3, args.warmup)):
+                fn()
+            ms = timed(torch, fn, args.steps, None) / args.steps
+            print(json.dumps({"layout": lname, "arm": arm, "requests": len(recs), "prompt_tokens_mean": float(ns.mean()),
+                              "hit_blocks": int(nc.sum()) // 16, "suffix_tokens": int((ns - nc).sum()), "attn_flops": flops,
+                              "predicted_docs": int(sum(rec.depth for rec in recs)),
+                              "matched_docs": int(sum(tracegen.docs_within(trace, rec.order, rec.n_cached) for rec in recs)),
+                              "prefill_ms": ms, "attn_tflops_incl_append": flops / ms / 1e9}), flush=True)
+            del q, k, v, qr, out
+
+
 def run_arms(args):
     """Ordering arms of the paper's Table 4 on the bench configuration: retrieval, sorted, recency,
     greedy (Algorithm 1), exhaustive.  One JSON line per arm with hit blocks, suffix tokens, attention flops, host admission
@@ -688,6 +735,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--skip-retrieval", action="store_true")
     ap.add_argument("--device-inputs", action="store_true", help="timing-only: draw q,k,v on the device (no e2e leg)")
+    ap.add_argument("--layouts", action="store_true", help="NEXT-3: paper-literal prompt layout vs the aligned plain layout, one JSON line per layout and arm")
     ap.add_argument("--mixed", action="store_true", help="NEXT-4: decode rows / prefill suffixes / both in one varlen launch, one JSON line each")
     ap.add_argument("--arms", action="store_true", help="ordering arms of the paper's Table 4 on --config, one JSON line per arm")
     ap.add_argument("--sweep", action="store_true", help="overlap x top-k sweep (BASELINE.json configs[2]), one JSON line per cell")
@@ -695,7 +743,9 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.oracle_requests is None:
         args.oracle_requests = {1: 4, 2: 16 if args.impl == "ours" else 4, 3: 4, 4: 1, 5: 1}[args.config]
-    if args.mixed:
+    if args.layouts:
+        run_layouts(args)
+    elif args.mixed:
         run_mixed(args)
     elif args.arms:
         run_arms(args)

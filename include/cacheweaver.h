@@ -63,7 +63,7 @@ typedef struct {
     /* predicted vs actual reusable prefix ("the trie can predict reuse for a path whose blocks were already
      * evicted"), summed over the requests admitted by cw_admit_batch and the calls of cw_feedback since cw_create/cw_reset: */
     int64_t predicted_prefix_docs;   /* sum of l(O,T)                                                        */
-    int64_t actual_prefix_docs;      /* sum of the documents lying entirely inside the matched tokens        */
+    int64_t actual_prefix_docs;      /* sum of the leading documents whose full 16-token blocks were all matched */
     int64_t over_predicted_docs;     /* sum of max(0, predicted - actual)                                    */
     int64_t stale_marks;             /* trie nodes marked stale (cw_mark_stale, cw_feedback, the residency-aware arm)  */
 } cw_stats_t;

@@ -336,8 +336,9 @@ int cw_admit_batch(cw_ctx* ctx, const int64_t* doc_ids, int32_t B, int32_t k, in
         if (rc == CW_ERR_NO_SPACE) return CW_OK;
         if (rc != CW_OK) return rc;
         for (int32_t i = nblk; i < max_blocks; ++i) table[i] = 0;
-        {   // predicted vs actual prefix: documents lying entirely inside the cached tokens
-            const int32_t actual = doc_len > 0 ? std::min<int32_t>(k, out_nc[r] / doc_len) : 0;
+        {   // predicted vs actual prefix: documents all of whose full 16-token blocks are inside the cached tokens
+            int32_t actual = 0;
+            while (actual < k && (int64_t)(actual + 1) * doc_len / CW_BLOCK_SIZE * CW_BLOCK_SIZE <= out_nc[r]) ++actual;
             if (reorder == CW_ARM_GREEDY_FEEDBACK || reorder == CW_ARM_GREEDY_RESIDENT) {
                 cw_feedback(ctx, O, k, out_pred[r], actual);
             } else {

@@ -88,7 +88,10 @@ class TraceRunner:
             O, depth = self.ctx.cw_order(D)
         elif self.strategy == "retrieval":
             O, depth = list(D), self.ctx.cw_predict(D)
-        else:                                              # sorted | recency | exhaustive (cw_order_arm)
+        elif self.cfg.layout != "plain":
+            raise ValueError("the token-based arms of cw_order_arm assemble docs ‖ query; use greedy / retrieval / "
+                             "greedy_feedback with the literal prompt layout")
+        else:                                              # sorted | recency | exhaustive | greedy_resident (cw_order_arm)
             O, depth = self.ctx.cw_order_arm(self.strategy, D, self.trace.doc_tokens, self.trace.query_tokens[r])
         tokens = tracegen.assemble_prompt(self.trace, r, O)
         req, table, c = self.ctx.cw_lookup(tokens)        # raises NoSpace with state unchanged
@@ -105,8 +108,7 @@ class TraceRunner:
 
         def close_wave():
             recs = [rec for _, rec in open_wave]
-            n = cfg.n
-            tables = np.zeros((len(recs), -(-n // BLOCK_SIZE)), dtype=np.int32)
+            tables = np.zeros((len(recs), max(len(rec.table) for rec in recs)), dtype=np.int32)
             for b, rec in enumerate(recs):
                 tables[b, : len(rec.table)] = rec.table
             s = np.array([len(rec.tokens) - rec.n_cached for rec in recs], dtype=np.int64)

@@ -23,6 +23,17 @@ import numpy as np
 
 BLOCK_SIZE = 16  # PAPER.md:39 "the token block size is 16 tokens"
 
+# Paper-literal prompt layout ("a fixed instruction, then the ordered evidence blocks
+# under [Document r: id] headers, then the query"; App. A).  There is no tokenizer here, so the template's
+# fixed strings are stood in for by reserved token ids outside the corpus vocabulary [0, 32000):
+#   instruction  INSTR_LEN seeded corpus-vocabulary tokens, the same for every request of a trace (~30 words in App. A)
+#   header(r, d) "[", "Document", rank r, ":", doc id d, "]", newline          -> HEADER_LEN tokens; contains the RANK
+#   separator    blank line after the document text                             -> SEP_LEN token
+#   query        "Question", ":", <query tokens>, newline, "Answer", ":"        -> QHEAD_LEN + q_len + QTAIL_LEN tokens
+INSTR_LEN, HEADER_LEN, SEP_LEN, QHEAD_LEN, QTAIL_LEN = 30, 7, 1, 2, 3
+T_LBRACKET, T_DOCUMENT, T_COLON, T_RBRACKET, T_NEWLINE, T_BLANKLINE, T_QUESTION, T_ANSWER = range(32000, 32008)
+T_RANK0, T_DOCID0 = 32100, 33000
+
 
 @dataclass(frozen=True)
 class Config:
@@ -44,9 +55,14 @@ class Config:
     n_clusters: int = 1
     zipf_s: float = 1.1
     admission: str = "sequential"   # "sequential" | "waves"
+    layout: str = "plain"    # "plain": docs ‖ query (north_star) | "literal": the paper's template (App. A), see segments()
+    doc_jitter: int = 0      # layout "literal": document lengths are drawn from U[doc_len - jitter, doc_len + jitter]
 
     @property
     def n(self) -> int:
+        """prompt length in tokens; for the literal layout (ragged documents) the largest possible one."""
+        if self.layout == "literal":
+            return INSTR_LEN + self.k * (HEADER_LEN + self.doc_len + self.doc_jitter + SEP_LEN) + QHEAD_LEN + self.q_len + QTAIL_LEN
         return self.k * self.doc_len + self.q_len
 
     @property
@@ -85,9 +101,11 @@ def config3(k: int, overlap_pct: int, n_req: int = 128) -> Config:
 @dataclass
 class Trace:
     cfg: Config
-    doc_tokens: np.ndarray              # int32 [total_docs, doc_len]
+    doc_tokens: np.ndarray              # int32 [total_docs, doc_len] (layout "literal": padded to the longest document)
     retrieval: list                     # n_req lists of int64 doc ids, in retrieval rank
     query_tokens: np.ndarray            # int32 [n_req, q_len]
+    doc_lens: np.ndarray | None = None  # int32 [total_docs], layout "literal" only
+    instr_tokens: np.ndarray | None = None   # int32 [INSTR_LEN], layout "literal" only
     _chunks: dict = field(default_factory=dict, repr=False)
 
 
@@ -95,7 +113,8 @@ def make_trace(cfg: Config) -> Trace:
     """Everything derived in a fixed order from one PCG64 generator seeded with cfg.seed."""
     rng = np.random.default_rng(cfg.seed)
     total_docs = cfg.n_docs * cfg.n_clusters
-    doc_tokens = rng.integers(0, 32000, size=(total_docs, cfg.doc_len), dtype=np.int32)
+    doc_tokens = rng.integers(0, 32000, size=(total_docs, cfg.doc_len + (cfg.doc_jitter if cfg.layout == "literal" else 0)),
+                              dtype=np.int32)
     retrieval = []
     if cfg.mode == "overlap":
         prev = None
@@ -120,6 +139,10 @@ def make_trace(cfg: Config) -> Trace:
     else:
         raise ValueError(cfg.mode)
     query_tokens = rng.integers(0, 32000, size=(cfg.n_req, cfg.q_len), dtype=np.int32)
+    if cfg.layout == "literal":      # drawn last, so the plain-layout traces of the same seed are unchanged
+        doc_lens = rng.integers(cfg.doc_len - cfg.doc_jitter, cfg.doc_len + cfg.doc_jitter + 1, size=total_docs).astype(np.int32)
+        instr = rng.integers(0, 32000, size=INSTR_LEN, dtype=np.int32)
+        return Trace(cfg, doc_tokens, retrieval, query_tokens, doc_lens, instr)
     return Trace(cfg, doc_tokens, retrieval, query_tokens)
 
 
@@ -129,22 +152,56 @@ def jaccard(a, b) -> float:
     return len(a & b) / len(a | b)
 
 
+def segments(trace: Trace, r, order):
+    """The prompt of request r under `order` as a list of (key, tokens) segments; the key names what the segment's
+    activations depend on (the document PREFIX for evidence blocks), r = None leaves the query segment out.
+      plain   : [doc O[0]] … [doc O[k-1]] [query]                                  (north_star: docs then query)
+      literal : [instruction] [header(1, O[0]) doc O[0] blank line] … [Question: query \n Answer:]   (App. A)"""
+    cfg = trace.cfg
+    i32 = lambda xs: np.asarray(xs, dtype=np.int32)
+    segs = []
+    if cfg.layout == "literal":
+        segs.append(((2,), trace.instr_tokens))
+        for j, d in enumerate(order):
+            d = int(d)
+            hdr = i32([T_LBRACKET, T_DOCUMENT, T_RANK0 + j + 1, T_COLON, T_DOCID0 + d, T_RBRACKET, T_NEWLINE])
+            segs.append(((0, *[int(x) for x in order[: j + 1]]),
+                         np.concatenate([hdr, trace.doc_tokens[d, : trace.doc_lens[d]], i32([T_BLANKLINE])])))
+        if r is not None:
+            segs.append(((1, int(r)), np.concatenate([i32([T_QUESTION, T_COLON]), trace.query_tokens[r],
+                                                      i32([T_NEWLINE, T_ANSWER, T_COLON])])))
+    else:
+        for j, d in enumerate(order):
+            segs.append(((0, *[int(x) for x in order[: j + 1]]), trace.doc_tokens[int(d)]))
+        if r is not None:
+            segs.append(((1, int(r)), trace.query_tokens[r]))
+    return segs
+
+
 def assemble_prompt(trace: Trace, r: int, order) -> np.ndarray:
-    """a3: tokens = doc_tokens[O[0]] ‖ … ‖ doc_tokens[O[k-1]] ‖ query_tokens[r] (north_star: docs then query)."""
-    parts = [trace.doc_tokens[d] for d in order] + [trace.query_tokens[r]]
-    return np.ascontiguousarray(np.concatenate(parts), dtype=np.int32)
+    """a3: the prompt tokens of request r with its documents in `order` (see segments())."""
+    return np.ascontiguousarray(np.concatenate([t for _, t in segments(trace, r, order)]), dtype=np.int32)
 
 
 def doc_prefix_tokens(trace: Trace, docs) -> np.ndarray:
-    """tokens of the prompt prefix made of the leading documents `docs` (no query): what a residency peek looks up."""
-    if len(docs) == 0:
+    """tokens of the prompt prefix that ends with the leading documents `docs` (no query): what a residency peek looks up."""
+    parts = [t for _, t in segments(trace, None, docs)]
+    if not parts:
         return np.zeros(0, dtype=np.int32)
-    return np.ascontiguousarray(np.concatenate([trace.doc_tokens[d] for d in docs]), dtype=np.int32)
+    return np.ascontiguousarray(np.concatenate(parts), dtype=np.int32)
 
 
 def docs_within(trace: Trace, order, n_tokens: int) -> int:
-    """number of leading documents of `order` that lie entirely inside the first n_tokens prompt tokens."""
-    return min(len(order), int(n_tokens) // trace.cfg.doc_len)
+    """number of leading documents of `order` covered by the first n_tokens prompt tokens: every FULL 16-token block up to
+    the end of the document's segment lies inside them (the block a document shares with what follows can never be
+    matched unless the next segment matches too; for block-aligned documents this is plain containment)."""
+    pos, m = 0, 0
+    for key, t in segments(trace, None, order):
+        pos += len(t)
+        if pos // BLOCK_SIZE * BLOCK_SIZE > n_tokens:
+            break
+        m += key[0] == 0
+    return m
 
 
 def f32_to_bf16_bits(x: np.ndarray) -> np.ndarray:
@@ -164,11 +221,13 @@ def _chunk(seed: int, key: tuple, length: int, width: int) -> np.ndarray:
 
 
 def qkv_chunk_keys(trace: Trace, r: int, order):
-    """(key, length) of each activation chunk of request r's prompt under `order`."""
-    cfg = trace.cfg
-    keys = [((0, *[int(d) for d in order[: j + 1]]), cfg.doc_len) for j in range(len(order))]
-    keys.append(((1, int(r)), cfg.q_len))
-    return keys
+    """(key, length) of each activation chunk of request r's prompt under `order` (one chunk per prompt segment)."""
+    if trace.cfg.layout == "plain":          # no token arrays needed: fixed lengths
+        cfg = trace.cfg
+        keys = [((0, *[int(d) for d in order[: j + 1]]), cfg.doc_len) for j in range(len(order))]
+        keys.append(((1, int(r)), cfg.q_len))
+        return keys
+    return [(key, len(t)) for key, t in segments(trace, r, order)]
 
 
 def prompt_qkv(trace: Trace, r: int, order, start: int = 0, cache: bool = False) -> np.ndarray:
