@@ -272,13 +272,17 @@ class OracleSample:
     configuration, greedy order, sequential: order/lookup/observe + RoPE + pool append + suffix attention + release.
     Inputs are generated before the timed region."""
 
-    def __init__(self, cfg_id, n_req):
+    def __init__(self, cfg_id, n_req, max_rows=None):
         from oracle.pipeline import run_trace
         self.cfg = cfg = tracegen.CONFIGS[cfg_id] if isinstance(cfg_id, int) else cfg_id
         self.trace = tracegen.make_trace(cfg)
         self.reqs = list(range(min(n_req, cfg.n_req)))
         dry = run_trace(self.trace, "greedy", compute=False, requests=self.reqs)
-        self.flops = attention_flops(cfg, [rr.n_cached for rr in dry.requests])
+        # max_rows bounds the sample further for the long prompts (cfg 5: one request is ~70 s of fp64 numpy): only the first
+        # max_rows suffix rows of each sampled request are prefilled (a prompt cut after n_cached + max_rows tokens)
+        self.max_rows = max_rows
+        self.flops = sum(4 * cfg.Hq * cfg.D * (m * (m + 1) // 2 - rr.n_cached * (rr.n_cached + 1) // 2)
+                         for rr in dry.requests for m in [min(cfg.n, rr.n_cached + (max_rows or cfg.n))])
         for rr in dry.requests:                       # warm tracegen's chunk cache: no RNG inside the timed region
             tracegen.prompt_qkv(self.trace, rr.r, rr.order, rr.n_cached, cache=True)
         self.dry = dry
@@ -296,6 +300,8 @@ class OracleSample:
             req, table, c = bm.lookup(tokens)
             tree.observe(O)
             rows = tracegen.prompt_qkv(trace, r, O, c, cache=True)
+            if self.max_rows:
+                rows = rows[:self.max_rows]
             q, k, v = (tracegen.bf16_bits_to_f64(x) for x in tracegen.split_qkv(cfg, rows))
             attention_suffix(pool, table, c, q, k, v, cfg.theta)
             bm.release(req)
@@ -312,14 +318,15 @@ def run_reference(args):
     rank, _, world = dist_env()
     if rank != 0:
         return
-    sample = OracleSample(select_config(args), args.oracle_requests)
+    sample = OracleSample(select_config(args), args.oracle_requests, args.oracle_rows)
     for _ in range(args.warmup):
         sample.run()
     times = [sample.run() for _ in range(args.steps)]
     total = sum(times)
     value = sample.flops * args.steps / total / 1e12
     cores = oracle_threads()
-    desc = f"first {len(sample.reqs)} of {sample.cfg.n_req} requests of {sample.cfg.name} per step, sequential, greedy order"
+    desc = f"first {len(sample.reqs)} of {sample.cfg.n_req} requests of {sample.cfg.name} per step, sequential, greedy order" + \
+           (f", first {sample.max_rows} suffix rows of each" if sample.max_rows else "")
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
@@ -449,9 +456,10 @@ def run_ours(args):
         prefill["arms_cfg1"] = cfg1_four_arms(device)
     cpu = None
     if world == 1 or rank == 0:
-        sample = OracleSample(cfg_sel, args.oracle_requests)
+        sample = OracleSample(cfg_sel, args.oracle_requests, args.oracle_rows)
         t = sample.run()
-        desc = f"first {len(sample.reqs)} of {cfg.n_req} requests of {cfg.name}, sequential, greedy order, one pass"
+        desc = f"first {len(sample.reqs)} of {cfg.n_req} requests of {cfg.name}, sequential, greedy order, one pass" + \
+               (f", first {sample.max_rows} suffix rows of each" if sample.max_rows else "")
         cpu = {"value": sample.flops / t / 1e12, "unit": UNIT, "cores": oracle_threads(), "kind": "oracle", "sample": desc,
                "seconds": t}
 
@@ -732,6 +740,7 @@ def main():
     ap.add_argument("--skip-per-request", action="store_true")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--oracle-requests", type=int, default=None, help="requests in the oracle's bounded sample")
+    ap.add_argument("--oracle-rows", type=int, default=None, help="suffix rows per request in the oracle's bounded sample")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--skip-retrieval", action="store_true")
     ap.add_argument("--device-inputs", action="store_true", help="timing-only: draw q,k,v on the device (no e2e leg)")
@@ -743,6 +752,8 @@ def main():
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.oracle_requests is None:
         args.oracle_requests = {1: 4, 2: 16 if args.impl == "ours" else 4, 3: 4, 4: 1, 5: 1}[args.config]
+    if args.oracle_rows is None and args.config == 5:
+        args.oracle_rows = 4096           # ~12 s instead of ~70 s for the whole 10 304-token prompt
     if args.layouts:
         run_layouts(args)
     elif args.mixed:
