@@ -49,6 +49,10 @@ typedef struct {
     void*   rope_table;      /* device, caller-owned, max_position*(D/2)*2 fp32 {cos,sin}; FILLED by cw_create.
                                 may be NULL together with k_pool/v_pool for a host-only context (no kernels) */
     int32_t device;          /* CUDA device ordinal (ignored for a host-only context)                       */
+    int32_t index_key_bits;  /* 0 or >= 64: the prefix index is keyed by the whole 64-bit chain hash; 1..63: by its low bits only.
+                                Every index entry is also checked against a second, secretly salted 64-bit chain, so a key
+                                collision (accidental or crafted) never serves another prompt's KV: the colliding block is just
+                                not cached.  Small values make collisions frequent (used by the tests of that property).     */
 } cw_config;
 
 typedef struct {
@@ -199,7 +203,10 @@ int cw_free_list(cw_ctx* ctx, int32_t* out, int32_t cap, int32_t* out_len);
  *     slot(p) = (block_table[p/16], p%16)          (DESIGN.md c4 split-half RoPE)
  *   q [T,Hq,D], k,v [T,Hkv,D]: device bf16, row-major contiguous.  q_roped: device bf16, T*Hq*D elements, request r
  *   owns the slice starting at cu_seqlens_q[r]*Hq*D, laid out as cw_q_roped_offset() says; it must NOT alias q
- *   (q is read through the non-coherent path).  Positions >= max_position are invalid.  The pools must have been
+ *   (q is read through the non-coherent path).  The descriptors are on the device, so they cannot be rejected by this call:
+ *   a token whose position is >= max_position or >= 16*max_blocks_per_req, or whose table entry is not in [0, NB), is
+ *   SKIPPED (nothing of it is written: no clamped rotation, no store outside the pool); cw_prefill_attn flags a request
+ *   that is too long in its work header.  The pools must have been
  *   zero-filled once by the caller (stale slots of a partially filled block must hold finite values). */
 int cw_append_kv(cw_ctx* ctx, const void* q, const void* k, const void* v, void* q_roped,
                  const int32_t* d_cu_seqlens_q, const int32_t* d_n_cached, const int32_t* d_block_tables,

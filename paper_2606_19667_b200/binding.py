@@ -24,7 +24,7 @@ class CwConfig(C.Structure):
                 ("num_kv_heads", C.c_int32), ("head_dim", C.c_int32), ("max_position", C.c_int32),
                 ("rope_theta", C.c_double), ("recency_window", C.c_int32), ("eager_register", C.c_int32),
                 ("hash_salt", C.c_uint64), ("k_pool", C.c_void_p), ("v_pool", C.c_void_p),
-                ("rope_table", C.c_void_p), ("device", C.c_int32)]
+                ("rope_table", C.c_void_p), ("device", C.c_int32), ("index_key_bits", C.c_int32)]
 
 
 class CwStats(C.Structure):
@@ -125,12 +125,12 @@ class Context:
     """One cw_ctx.  device=None -> host-only context (ordering + prefix cache, no kernels, no CUDA needed)."""
 
     def __init__(self, num_blocks, num_q_heads, num_kv_heads, head_dim, recency_window, rope_theta=10000.0,
-                 max_position=0, eager_register=True, hash_salt=0, device=None):
+                 max_position=0, eager_register=True, hash_salt=0, device=None, index_key_bits=0):
         self.lib = load_library()
         self.device = device
         self.Hq, self.Hkv, self.D, self.NB = num_q_heads, num_kv_heads, head_dim, num_blocks
         cfg = CwConfig(BLOCK_SIZE, num_blocks, num_q_heads, num_kv_heads, head_dim, max_position, float(rope_theta),
-                       recency_window, int(bool(eager_register)), hash_salt, None, None, None, 0)
+                       recency_window, int(bool(eager_register)), hash_salt, None, None, None, 0, int(index_key_bits))
         self.k_pool = self.v_pool = self.rope_table = None
         if device is not None:
             import torch

@@ -78,7 +78,7 @@ int cw_create(const cw_config* cfg, cw_ctx** out) {
     ctx->host_only = host_only;
     ctx->num_sms = 148;
     ctx->tree = new cw::KnowledgeTree(cfg->recency_window);
-    ctx->blocks = new cw::BlockManager(cfg->num_blocks, cfg->eager_register != 0, cfg->hash_salt);
+    ctx->blocks = new cw::BlockManager(cfg->num_blocks, cfg->eager_register != 0, cfg->hash_salt, cfg->index_key_bits);
     if (!host_only) {
         cudaError_t e = cudaSetDevice(cfg->device);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, cfg->device);
@@ -227,14 +227,14 @@ int cw_order_arm(cw_ctx* ctx, int32_t arm, const int64_t* doc_ids, int32_t k, co
         if (q_len) std::memcpy(tokens.data() + (size_t)k * doc_len, query_tokens, sizeof(int32_t) * (size_t)q_len);
         std::vector<int> perm((size_t)k);
         for (int i = 0; i < k; ++i) perm[(size_t)i] = i;
-        std::vector<uint64_t> chain;
+        std::vector<uint64_t> chain, vchain;
         int32_t best = -1;
         do {   // permutations in lexicographic order of retrieval-rank indices; keep the first maximiser
             for (int i = 0; i < k; ++i)
                 std::memcpy(tokens.data() + (size_t)i * doc_len, doc_tokens + (size_t)doc_ids[perm[(size_t)i]] * doc_len,
                             sizeof(int32_t) * (size_t)doc_len);
-            ctx->blocks->chain(tokens.data(), n, chain);
-            const int32_t m = ctx->blocks->match(chain, n);
+            ctx->blocks->chains(tokens.data(), n, chain, vchain);
+            const int32_t m = ctx->blocks->match(chain, vchain, n);
             if (m > best) {
                 best = m;
                 for (int i = 0; i < k; ++i) out_order[i] = doc_ids[perm[(size_t)i]];
@@ -260,8 +260,9 @@ int cw_lookup(cw_ctx* ctx, const int32_t* tokens, int32_t n, int32_t peek_only, 
     if (!ctx || !tokens || n <= 0 || !out_n_cached) return fail(ctx, CW_ERR_INVALID, "cw_lookup: bad argument");
     if (peek_only) {
         std::vector<uint64_t> ch;
-        ctx->blocks->chain(tokens, n, ch);
-        *out_n_cached = ctx->blocks->match(ch, n) * CW_BLOCK_SIZE;
+        std::vector<uint64_t> vc;
+        ctx->blocks->chains(tokens, n, ch, vc);
+        *out_n_cached = ctx->blocks->match(ch, vc, n) * CW_BLOCK_SIZE;
         return CW_OK;
     }
     if (!out_req || !out_block_table) return fail(ctx, CW_ERR_INVALID, "cw_lookup: null output");
@@ -287,7 +288,8 @@ int cw_reset(cw_ctx* ctx) {
     delete ctx->tree;
     delete ctx->blocks;
     ctx->tree = new cw::KnowledgeTree(ctx->cfg.recency_window);
-    ctx->blocks = new cw::BlockManager(ctx->cfg.num_blocks, ctx->cfg.eager_register != 0, ctx->cfg.hash_salt);
+    ctx->blocks = new cw::BlockManager(ctx->cfg.num_blocks, ctx->cfg.eager_register != 0, ctx->cfg.hash_salt,
+                                       ctx->cfg.index_key_bits);
     ctx->last_served.clear();
     ctx->last_error.clear();
     ctx->pred_docs = ctx->actual_docs = ctx->over_pred_docs = 0;

@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(THREADS) append_kv_kernel(
     const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ k, const __nv_bfloat16* __restrict__ v,
     __nv_bfloat16* __restrict__ q_roped, __nv_bfloat16* __restrict__ k_pool, __nv_bfloat16* __restrict__ v_pool,
     const float* __restrict__ rope_table, const int32_t* __restrict__ cu, const int32_t* __restrict__ ncached,
-    const int32_t* __restrict__ tables, int max_blocks, int B, int T, int Hq, int Hkv, int max_position) {
+    const int32_t* __restrict__ tables, int max_blocks, int B, int T, int Hq, int Hkv, int max_position, int num_blocks) {
     constexpr int CPH = D / 16;                       // chunk pairs (units) per head
     const int g = Hq / Hkv, tpt = 128 / g;
     const int uq = Hq * CPH, uk = Hkv * CPH;
@@ -80,9 +80,14 @@ __global__ void __launch_bounds__(THREADS) append_kv_kernel(
         const int qt = tl / tpt, tloc = tl - qt * tpt;
         const int rows_valid = min(tpt, s_len - qt * tpt) * g;
         const size_t q_tile_base = (size_t)q_begin * Hq * D + (size_t)qt * (tpt * g) * D;
-        const int blk = __ldg(tables + (size_t)r * max_blocks + (p >> 4));
+        // A token whose position has no RoPE row or no table slot, or whose table entry is not a pool block, is skipped: nothing
+        // of it is written (no clamping to a wrong rotation, no store outside the pool).  cw_prefill_attn reports a request
+        // that is too long through its error flag.
+        const bool pos_ok = p >= 0 && p < max_position && (p >> 4) < max_blocks;
+        const int blk = pos_ok ? __ldg(tables + (size_t)r * max_blocks + (p >> 4)) : -1;
+        if (blk < 0 || blk >= num_blocks) continue;
         const int tib = p & 15;
-        const int prow = p < max_position ? p : max_position - 1;
+        const int prow = p;
         // A thread's units are THREADS apart and THREADS % CPH == 0, so all of them rotate the same 8 frequencies: the
         // {cos, sin} pairs are loaded once per token and thread (they would otherwise double the L1 load traffic).
         static_assert(THREADS % CPH == 0, "chunk index must be the same for every unit of a thread");
@@ -159,7 +164,7 @@ int launch_append_kv(const cw_config& cfg, const void* q, const void* k, const v
     append_kv_kernel<DD, TT><<<(unsigned)grid, TT, 0, s>>>(                                                               \
         (const __nv_bfloat16*)q, (const __nv_bfloat16*)k, (const __nv_bfloat16*)v, (__nv_bfloat16*)q_roped,     \
         (__nv_bfloat16*)cfg.k_pool, (__nv_bfloat16*)cfg.v_pool, (const float*)cfg.rope_table, cu, ncached,      \
-        tables, max_blocks, B, T, cfg.num_q_heads, cfg.num_kv_heads, cfg.max_position)
+        tables, max_blocks, B, T, cfg.num_q_heads, cfg.num_kv_heads, cfg.max_position, cfg.num_blocks)
 #define CW_LAUNCH_APPEND_D(DD)                                                                                  \
     do {                                                                                                        \
         if (threads == 128) { CW_LAUNCH_APPEND(DD, 128); }                                                      \

@@ -69,6 +69,7 @@ class KnowledgeTree {
 struct Request {
     std::vector<int32_t> table;
     std::vector<uint64_t> chain;
+    std::vector<uint64_t> verify;  // second, secretly salted chain over the same blocks (collision check, see BlockManager)
     int32_t m;      // matched (cached) blocks
     int32_t n;      // sequence length in tokens (prompt + what cw_extend appended)
     int32_t n_done; // tokens whose K/V are (being) written to the pool: m*16 at lookup, advanced by cw_prefill_requests
@@ -77,18 +78,23 @@ struct Request {
 
 class BlockManager {
   public:
-    BlockManager(int32_t num_blocks, bool eager, uint64_t salt);
+    BlockManager(int32_t num_blocks, bool eager, uint64_t salt, int32_t key_bits = 64);
     void chain(const int32_t* tokens, int32_t n, std::vector<uint64_t>& out) const;
-    int32_t match(const std::vector<uint64_t>& chain, int32_t n) const;
+    // Both chains of a token sequence: `h` is the FNV-1a-64 chain that keys the prefix index (reading c2), `v` an
+    // independent 64-bit chain (multiply-xorshift mixing) salted with a per-context random secret.  An index entry only
+    // matches when BOTH agree, so serving another prompt's KV needs a simultaneous collision of two unrelated functions, one of
+    // them keyed with a value the prompt author cannot know; a colliding newcomer is simply never cached.
+    void chains(const int32_t* tokens, int32_t n, std::vector<uint64_t>& h, std::vector<uint64_t>& v) const;
+    int32_t match(const std::vector<uint64_t>& h, const std::vector<uint64_t>& v, int32_t n) const;
     // NEXT-1 peek, incremental over a growing document prefix: state = (hash of the last full block, tokens of the
     // pending partial block).  extend() appends tokens; it returns false and leaves the state unchanged unless every
     // full block completed by them is resident.
     struct Probe {
-        uint64_t parent;
+        uint64_t parent, vparent;
         int32_t pending[CW_BLOCK_SIZE];
         int32_t n_pending;
     };
-    Probe probe_begin() const { return Probe{salt_, {0}, 0}; }
+    Probe probe_begin() const { return Probe{salt_, vsalt_, {0}, 0}; }
     bool probe_extend(Probe& p, const int32_t* tokens, int32_t n) const;
     // returns CW_OK / CW_ERR_NO_SPACE
     int lookup(const int32_t* tokens, int32_t n, int64_t* req, int32_t* table, int32_t* n_cached);
@@ -111,12 +117,14 @@ class BlockManager {
     void unlink(int32_t b);
     void push_tail(int32_t b);
     void reg(const Request& r, int32_t nfull);
+    int32_t find_block(uint64_t h, uint64_t v) const;   // block registered under (h, v), or -1
     int32_t NB_;
     bool eager_;
-    uint64_t salt_;
+    uint64_t salt_, vsalt_, key_mask_;
+    uint64_t key(uint64_t h) const { return h & key_mask_; }
     std::vector<int32_t> ref_, prev_, next_;   // list nodes 0..NB-1, sentinel = NB
     std::vector<uint8_t> has_hash_;
-    std::vector<uint64_t> hash_;
+    std::vector<uint64_t> hash_, verify_;
     std::unordered_map<uint64_t, int32_t> index_;
     std::unordered_map<int64_t, Request> reqs_;
     int64_t next_req_ = 1;

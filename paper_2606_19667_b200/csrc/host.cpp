@@ -6,6 +6,7 @@
 #include <algorithm>
 #include <climits>
 #include <cstring>
+#include <random>
 
 namespace cw {
 
@@ -101,9 +102,11 @@ void KnowledgeTree::prune() {
 // --------------------------------------------------------------------------------------- block manager ----
 static inline uint64_t fnv1a_step(uint64_t h, uint8_t byte) { return (h ^ byte) * 0x100000001B3ull; }
 
-BlockManager::BlockManager(int32_t num_blocks, bool eager, uint64_t salt)
-    : NB_(num_blocks), eager_(eager), salt_(salt), ref_(num_blocks, 0), prev_(num_blocks + 1), next_(num_blocks + 1),
-      has_hash_(num_blocks, 0), hash_(num_blocks, 0), free_count_(num_blocks) {
+BlockManager::BlockManager(int32_t num_blocks, bool eager, uint64_t salt, int32_t key_bits)
+    : NB_(num_blocks), eager_(eager), salt_(salt), key_mask_(key_bits <= 0 || key_bits >= 64 ? ~0ull : (1ull << key_bits) - 1), ref_(num_blocks, 0), prev_(num_blocks + 1), next_(num_blocks + 1),
+      has_hash_(num_blocks, 0), hash_(num_blocks, 0), verify_(num_blocks, 0), free_count_(num_blocks) {
+    std::random_device rd;
+    vsalt_ = ((uint64_t)rd() << 32) ^ (uint64_t)rd() ^ 0xA0761D6478BD642Full;
     // circular list with sentinel NB: head = next_[NB], tail = prev_[NB]; initial order 0,1,...,NB-1
     for (int32_t b = 0; b <= NB_; ++b) {
         next_[b] = (b + 1) % (NB_ + 1);
@@ -134,6 +137,17 @@ static inline uint64_t block_hash(uint64_t parent, const int32_t* tokens) {
     return h;
 }
 
+// verification chain: multiply-xorshift mixing of the parent value and the 16 tokens (unrelated to FNV-1a)
+static inline uint64_t verify_hash(uint64_t parent, const int32_t* tokens) {
+    uint64_t x = parent ^ 0x9E3779B97F4A7C15ull;
+    for (int t = 0; t < CW_BLOCK_SIZE; ++t) {
+        x = (x ^ (uint32_t)tokens[t]) * 0xFF51AFD7ED558CCDull;
+        x ^= x >> 32;
+    }
+    x *= 0xC4CEB9FE1A85EC53ull;
+    return x ^ (x >> 29);
+}
+
 // h_i = FNV1a64(LE64(h_{i-1}) || LE32(tok[16i]) ... LE32(tok[16i+15])), h_{-1} = salt  (DESIGN.md c2)
 void BlockManager::chain(const int32_t* tokens, int32_t n, std::vector<uint64_t>& out) const {
     int32_t nfull = n / CW_BLOCK_SIZE;
@@ -142,13 +156,30 @@ void BlockManager::chain(const int32_t* tokens, int32_t n, std::vector<uint64_t>
     for (int32_t i = 0; i < nfull; ++i) out[(size_t)i] = parent = block_hash(parent, tokens + (size_t)i * CW_BLOCK_SIZE);
 }
 
+void BlockManager::chains(const int32_t* tokens, int32_t n, std::vector<uint64_t>& h, std::vector<uint64_t>& v) const {
+    int32_t nfull = n / CW_BLOCK_SIZE;
+    h.resize((size_t)nfull);
+    v.resize((size_t)nfull);
+    uint64_t parent = salt_, vparent = vsalt_;
+    for (int32_t i = 0; i < nfull; ++i) {
+        h[(size_t)i] = parent = block_hash(parent, tokens + (size_t)i * CW_BLOCK_SIZE);
+        v[(size_t)i] = vparent = verify_hash(vparent, tokens + (size_t)i * CW_BLOCK_SIZE);
+    }
+}
+
+int32_t BlockManager::find_block(uint64_t h, uint64_t v) const {
+    auto it = index_.find(key(h));
+    return it != index_.end() && verify_[(size_t)it->second] == v ? it->second : -1;
+}
+
 bool BlockManager::probe_extend(Probe& p, const int32_t* tokens, int32_t n) const {
     Probe q = p;
     for (int32_t i = 0; i < n; ++i) {
         q.pending[q.n_pending++] = tokens[i];
         if (q.n_pending == CW_BLOCK_SIZE) {
             q.parent = block_hash(q.parent, q.pending);
-            if (!index_.count(q.parent)) return false;
+            q.vparent = verify_hash(q.vparent, q.pending);
+            if (find_block(q.parent, q.vparent) < 0) return false;
             q.n_pending = 0;
         }
     }
@@ -156,34 +187,35 @@ bool BlockManager::probe_extend(Probe& p, const int32_t* tokens, int32_t n) cons
     return true;
 }
 
-int32_t BlockManager::match(const std::vector<uint64_t>& ch, int32_t n) const {
+int32_t BlockManager::match(const std::vector<uint64_t>& ch, const std::vector<uint64_t>& vc, int32_t n) const {
     int32_t cap = (n - 1) / CW_BLOCK_SIZE, m = 0;
-    while (m < cap && index_.count(ch[(size_t)m])) ++m;
+    while (m < cap && find_block(ch[(size_t)m], vc[(size_t)m]) >= 0) ++m;
     return m;
 }
 
 void BlockManager::reg(const Request& r, int32_t nfull) {
     for (int32_t i = r.m; i < nfull; ++i) {
-        auto ins = index_.emplace(r.chain[(size_t)i], r.table[(size_t)i]);
-        if (ins.second) {
+        auto ins = index_.emplace(key(r.chain[(size_t)i]), r.table[(size_t)i]);
+        if (ins.second) {          // else: the same content is registered already, or a colliding block is (never cached)
             has_hash_[(size_t)r.table[(size_t)i]] = 1;
-            hash_[(size_t)r.table[(size_t)i]] = r.chain[(size_t)i];
+            hash_[(size_t)r.table[(size_t)i]] = key(r.chain[(size_t)i]);
+            verify_[(size_t)r.table[(size_t)i]] = r.verify[(size_t)i];
         }
     }
 }
 
 int BlockManager::lookup(const int32_t* tokens, int32_t n, int64_t* req, int32_t* table, int32_t* n_cached) {
     Request r;
-    chain(tokens, n, r.chain);
+    chains(tokens, n, r.chain, r.verify);
     int32_t nblk = (n + CW_BLOCK_SIZE - 1) / CW_BLOCK_SIZE, nfull = n / CW_BLOCK_SIZE;
     r.n = n;
     std::memcpy(r.tail, tokens + (size_t)nfull * CW_BLOCK_SIZE, sizeof(int32_t) * (size_t)(n - nfull * CW_BLOCK_SIZE));
-    r.m = match(r.chain, n);                                                    // (1)
+    r.m = match(r.chain, r.verify, n);                                          // (1)
     r.n_done = r.m * CW_BLOCK_SIZE;
     r.table.resize((size_t)nblk);
     int32_t matched_free = 0;
     for (int32_t i = 0; i < r.m; ++i) {
-        int32_t b = index_.find(r.chain[(size_t)i])->second;
+        int32_t b = index_.find(key(r.chain[(size_t)i]))->second;
         r.table[(size_t)i] = b;
         if (ref_[(size_t)b] == 0) ++matched_free;
     }
@@ -239,12 +271,14 @@ int BlockManager::extend(int64_t req, const int32_t* tokens, int32_t n_new, int3
     }
     const int32_t old_full = (int32_t)r.chain.size();
     int32_t n_tail = r.n - old_full * CW_BLOCK_SIZE;
-    uint64_t parent = old_full ? r.chain.back() : salt_;
+    uint64_t parent = old_full ? r.chain.back() : salt_, vparent = old_full ? r.verify.back() : vsalt_;
     for (int32_t i = 0; i < n_new; ++i) {
         r.tail[n_tail++] = tokens[i];
         if (n_tail == CW_BLOCK_SIZE) {
             parent = block_hash(parent, r.tail);
+            vparent = verify_hash(vparent, r.tail);
             r.chain.push_back(parent);
+            r.verify.push_back(vparent);
             n_tail = 0;
         }
     }

@@ -169,6 +169,48 @@ def test_append_kv_position_zero_is_identity(dev):
         assert np.array_equal(out_bits[0, h], b.v[0][0, h // g])
 
 
+def test_append_kv_skips_tokens_with_invalid_descriptors(dev):
+    """cacheweaver.h (cw_append_kv): the descriptors live on the device, so a bad one cannot be rejected by the call; a token
+    whose table entry is not a pool block, or whose position has no RoPE row / no table slot, must write NOTHING (no store
+    outside the pool, no rotation by a clamped position), and every other token is written as usual."""
+    Hq, Hkv, D = 8, 2, 128
+    b = Batch(dev, Hq, Hkv, D, cs=[0, 0, 0], ss=[40, 33, 20], seed=11)
+    for r in range(3):                              # unused table slots: not a block either (the Batch helper pads with 0)
+        b.tables[r, -(-b.ns[r] // 16):] = -1
+    good = b.tables.copy()
+    b.tables[1, 1] = b.ctx.NB + 7                   # request 1, positions 16..31: not a pool block
+    b.tables[2, 0] = -1                             # request 2, positions 0..15: negative id
+    b.d_tables = torch.from_numpy(b.tables).to(dev)
+    kp0, vp0 = b.ctx.k_pool.clone(), b.ctx.v_pool.clone()          # zero-filled pools
+    qr, cu, nc, d_cu, d_nc, T = b._append([0, 0, 0], b.ns)
+    # a second launch whose positions run past max_position (= 40) and past the table (3 blocks = 48 positions)
+    d_nc2 = torch.from_numpy(np.asarray([30, 30, 30], dtype=np.int32)).to(dev)
+    kp1, vp1 = b.ctx.k_pool.clone(), b.ctx.v_pool.clone()
+    b.ctx.cw_append_kv(*(to_dev(np.concatenate(x, axis=0), dev) for x in (b.q, b.k, b.v)), torch.empty_like(qr), d_cu, d_nc2,
+                       b.d_tables, b.max_blocks, b.B, T)
+    torch.cuda.synchronize()
+    f = tracegen.bf16_bits_to_f64
+    kp, vp = to_bits(kp1), to_bits(vp1)
+    for r in range(3):
+        k_ref = oattn.rope(f(b.k[r]), np.arange(b.ns[r]), b.theta)
+        for p in range(b.ns[r]):
+            skipped = (r == 1 and 16 <= p < 32) or (r == 2 and p < 16)
+            blk = int(good[r, p // 16])
+            off = b.ctx.cw_pool_offset(blk, 1, p % 16, 5)
+            if skipped:       # the block the table SHOULD have named was never touched
+                assert kp[off] == 0 and vp[off] == 0
+            else:
+                assert abs(tracegen.bf16_bits_to_f64(kp[off:off + 1])[0] - k_ref[p, 1, 5]) <= 2 ** -6 * max(1.0, abs(k_ref[p, 1, 5]))
+                assert vp[off] == b.v[r][p, 1, 5]
+    # second launch: positions 30..39 are valid for every request and rewritten with other rows' data; positions >= 40 skipped.
+    # What matters here: it ran without a fault and left every block of the pool that no valid (request, position) names alone.
+    used = {int(good[r, p // 16]) for r in range(3) for p in range(b.ns[r])}
+    kp2 = to_bits(b.ctx.k_pool).reshape(b.ctx.NB, -1)
+    for blk in range(b.ctx.NB):
+        if blk not in used:
+            assert not kp2[blk].any(), f"block {blk} is in no table but was written"
+
+
 # ---- kernel 2: varlen paged causal GQA attention ----------------------------------------------------------
 @pytest.mark.parametrize("Hq,Hkv,D,cs,ss", [
     (2, 1, 64, [0], [224]),                                  # cfg-1 shape, cold

@@ -326,3 +326,42 @@ def test_extend_matches_oracle_under_random_growth(seed):
         obm.check_invariants()
     st = ctx.cw_stats()
     assert (st["hit_blocks"], st["miss_blocks"], st["evictions"]) == (obm.hit_blocks, obm.miss_blocks, obm.evictions)
+
+
+@pytest.mark.parametrize("bits,eager", [(1, True), (3, True), (3, False), (6, True)])
+def test_index_key_collisions_never_serve_foreign_blocks(bits, eager):
+    """The prefix index keyed by only `bits` bits of the chain hash collides constantly.  Property (cacheweaver.h,
+    index_key_bits): a block returned as a hit for position i holds exactly this prompt's tokens [0, 16(i+1)) — checked
+    against a test-side record of what every block was allocated for — and the library never reports more cached blocks
+    than the oracle, which matches by token-prefix identity; with the full 64-bit key it reports the same."""
+    rng = random.Random(bits * 2 + eager)
+    nrng = np.random.default_rng(bits)
+    NB = 48
+    lib = Context(NB, 2, 1, 64, 4, eager_register=eager, index_key_bits=bits)
+    full = Context(NB, 2, 1, 64, 4, eager_register=eager)
+    docs = [nrng.integers(0, 30, 16 * rng.randint(1, 3), dtype=np.int32) for _ in range(9)]
+    content = {}                      # block id -> bytes of the token prefix it was allocated for
+    live, fewer = [], 0
+    for step in range(400):
+        if live and (rng.random() < 0.5 or len(live) > 2):
+            for h, x in zip((lib, full), live.pop(rng.randrange(len(live)))[:2]):
+                h.cw_release(x)
+            continue
+        O = rng.sample(range(len(docs)), rng.randint(1, 3))
+        toks = np.concatenate([docs[d] for d in O] + [nrng.integers(0, 30, rng.randint(1, 20), dtype=np.int32)])
+        raw = toks.astype("<i4").tobytes()
+        try:
+            req, tab, nc = lib.cw_lookup(toks)
+        except NoSpace:
+            continue
+        rf, tf, ncf = full.cw_lookup(toks)
+        live.append((req, rf))
+        for i, b in enumerate(tab.tolist()):
+            pre = raw[: 64 * (i + 1)]
+            if i < nc // 16:
+                assert content.get(b) == pre, f"step {step}: hit block {b} at position {i} holds another prefix"
+            else:
+                content[b] = pre if 16 * (i + 1) <= len(toks) else None      # partial last block: never matched
+        assert nc <= ncf
+        fewer += nc < ncf
+    assert fewer > 0, "the truncated key never collided: the test exercises nothing"
