@@ -357,6 +357,39 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 gn = geo_of(fetch(n_item + 1));
                 while (gq - gp < 2u && qk_step()) {}
                 for (int j = 0; j < gc.nt; ++j) {
+                    // Steady state (the interior chunks of an item: both cursors inside the item, Q K^T exactly two full chunks
+                    // ahead, nothing to open or close): one straight-line step — the issuing thread is the serial resource of a
+                    // tile (~5 clk per dependent instruction), so the general path below, which re-derives every case, would make
+                    // it the bottleneck of the whole kernel.
+                    if (j > 0 && !q_on_next && qj == j + 2 && qj + 1 < gc.n && gq - gp == 2u && (qj + 1) * kChunk <= gc.nkv) {
+                        const uint32_t b = pc & 1u;                                   // == sc & 1: S(j+2) replaces P(j)
+                        ptx::mbar_wait(bar(BAR_RING + vslot), vph);
+                        ptx::mbar_wait(bar(BAR_P_FULL + W * 2 + (int)b), (pc >> 1) & 1u);
+                        ptx::mbar_wait(bar(BAR_RING + kslot), kph);
+                        ptx::tc_fence_after();
+                        ptx::umma_ts_pv4<D>(tO, tS + b * 64u, vdesc0 + (uint64_t)((vslot * L::kKVBytes) >> 4), kIdescPV, 1u);
+                        ptx::umma_commit(bar(BAR_RING + NS + vslot));
+                        ptx::umma_ss_qk<D>(tS + b * 64u, qdesc, kdesc0 + (uint64_t)((kslot * L::kKVBytes) >> 4),
+                                           kIdescQK | ((uint32_t)(kChunk / 8) << 17));
+                        ptx::umma_commit(bar(BAR_S_FULL + W * 2 + (int)b));
+                        ptx::umma_commit(bar(BAR_RING + NS + kslot));
+                        ++pc;
+                        ++sc;
+                        ++gp;
+                        ++gq;
+                        ++qj;
+                        vslot += 2;
+                        if (vslot >= (uint32_t)NS) {
+                            vslot -= NS;
+                            vph ^= 1u;
+                        }
+                        kslot += 2;
+                        if (kslot >= (uint32_t)NS) {
+                            kslot -= NS;
+                            kph ^= 1u;
+                        }
+                        continue;
+                    }
                     // ---- O_w (+)= P_w[pc & 1] V(j) ----
                     ptx::mbar_wait(bar(BAR_RING + vslot), vph);
                     if (j < gc.n) {
@@ -424,25 +457,29 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
                 ptx::tc_fence_after();
                 const uint32_t tO = tmem + 256u + (uint32_t)t * 128u + lane_base;
                 __nv_bfloat16* orow = out + ((size_t)(w.tok0 + t * tpt + tdiv) * Hq + (size_t)w.kvh * g + hh) * D;
+                // O -> registers as packed bf16 (D/2 registers); the accumulator is handed back to the MMA warp as soon as it has
+                // been READ — the global stores, which are what takes time here, run while the next item's P V accumulates
+                uint32_t pk[D / 2];
 #pragma unroll
                 for (int i = 0; i < D / 32; ++i) {
                     uint32_t o[32];
                     ptx::tmem_ld32(tO + i * 32, o);
                     ptx::tmem_ld_wait();
-                    if (row_valid) {
 #pragma unroll
-                        for (int e = 0; e < 32; e += 8) {
-                            uint4 pk;
-                            pk.x = ptx::pack_bf16x2(__uint_as_float(o[e]) * inv_l, __uint_as_float(o[e + 1]) * inv_l);
-                            pk.y = ptx::pack_bf16x2(__uint_as_float(o[e + 2]) * inv_l, __uint_as_float(o[e + 3]) * inv_l);
-                            pk.z = ptx::pack_bf16x2(__uint_as_float(o[e + 4]) * inv_l, __uint_as_float(o[e + 5]) * inv_l);
-                            pk.w = ptx::pack_bf16x2(__uint_as_float(o[e + 6]) * inv_l, __uint_as_float(o[e + 7]) * inv_l);
-                            *reinterpret_cast<uint4*>(orow + i * 32 + e) = pk;
-                        }
-                    }
+                    for (int x = 0; x < 16; ++x)
+                        pk[i * 16 + x] = ptx::pack_bf16x2(__uint_as_float(o[2 * x]) * inv_l, __uint_as_float(o[2 * x + 1]) * inv_l);
                 }
                 ptx::tc_fence_before();
                 ptx::mbar_arrive(bar(BAR_O_EMPTY + t));
+                if (row_valid) {
+                    // one thread owns one row: 32-byte stores (a whole sector each; a 16-byte store touches the same number of
+                    // sectors for half the bytes)
+#pragma unroll
+                    for (int e = 0; e < D / 2; e += 8) {
+                        const uint32_t v8[8] = {pk[e], pk[e + 1], pk[e + 2], pk[e + 3], pk[e + 4], pk[e + 5], pk[e + 6], pk[e + 7]};
+                        ptx::st_global_v8(orow + 2 * e, v8);
+                    }
+                }
             }
         }
     } else {
