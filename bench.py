@@ -409,7 +409,7 @@ def run_ours(args):
     # end to end: host buffers, H2D/D2H inside the timed region
     e2e_steps, ms_e2e, e2e_value = 0, None, None
     if not args.device_inputs:
-        for _ in range(max(1, args.warmup // 2)):
+        for _ in range(max(2, args.warmup // 2)):
             wl.step_e2e()
         wl.h2d = wl.d2h = 0
         e2e_steps = max(1, min(args.steps, args.e2e_steps))
