@@ -15,10 +15,12 @@
 // warp-specialised, mbarrier pipelines only:
 //   warps 0-3   softmax of Q tile 0 (thread i owns TMEM lane i = packed row i)
 //   warps 4-7   the same for Q tile 1
-//   warps 8-11  epilogue of both tiles: O_w / l_w -> bf16 -> global, so the softmax groups go straight on to the next item
-//   warp  12    MMA issuer (one elected lane): S_w[b] = Q_w K(j)^T (SS, N = 64) and O_w += P_w[b] V(j) (TS: P is read from
-//               TMEM); the chunk streams of consecutive items are chained (the first two QK^T of the next item are issued
-//               behind the last PVs of the current one); owns TMEM alloc/dealloc (512 columns: S0a S0b S1a S1b O0 O1)
+//   warps 8-11  epilogue of both tiles: O_w / l_w -> packed bf16 in registers, accumulator handed back, 32-byte stores; the
+//               softmax groups go straight on to the next item
+//   warps 12,14 MMA issuers of Q tile 0 / 1 (one elected lane each): S_w[b] = Q_w K(j)^T (SS, N = 64) and O_w += P_w[b] V(j)
+//               (TS: P is read from TMEM); the chunk streams of consecutive items are chained (the first two QK^T of the
+//               next item are issued behind the last PVs of the current one); interior chunks take a straight-line step;
+//               warp 12 owns TMEM alloc/dealloc (512 columns: S0a S0b S1a S1b O0 O1)
 //   warp  13    loader: Q tiles (q_roped is stored tile-packed and pre-swizzled by cw_append_kv: one bulk copy per
 //               64-dim half tile) and K/V chunks (one bulk copy per 16-token pool block per operand, gathered through
 //               the block table; pool blocks are pre-swizzled in the UMMA canonical layout) into a multi-stage ring
