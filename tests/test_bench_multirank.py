@@ -53,3 +53,19 @@ def test_reference_arm_prints_on_rank_zero_only():
     d = lines[0]
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["cpu_baseline"]["kind"] == "oracle"
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["value"] > 0 and d["unit"] == "TFLOP/s"
+
+
+def test_oracle_sample_with_row_bound_counts_the_rows_it_computes():
+    """bench.py's bounded oracle sample (`--oracle-rows`, default for config 5): the flops it reports are those of the
+    rows the oracle really computes — a prompt cut after n_cached + max_rows tokens — and the full sample is unchanged."""
+    sys.path.insert(0, ROOT)
+    import bench
+    import tracegen
+    cfg = tracegen.CONFIGS[1]
+    full = bench.OracleSample(1, 2)
+    cut = bench.OracleSample(1, 2, max_rows=40)
+    ncs = [rr.n_cached for rr in full.dry.requests]
+    assert full.flops == bench.attention_flops(cfg, ncs)
+    want = sum(4 * cfg.Hq * cfg.D * sum(p + 1 for p in range(c, min(cfg.n, c + 40))) for c in ncs)
+    assert cut.flops == want and cut.flops < full.flops
+    assert cut.run() > 0 and full.run() > 0
