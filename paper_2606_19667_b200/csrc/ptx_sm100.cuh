@@ -172,9 +172,9 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi), "f"(lo));
     return r;
 }
-// 256-bit global store (sm_100: STG.256), 32-byte aligned
+// 256-bit global store (sm_100: STG.256), 32-byte aligned, not allocated in L1 (the line is written once)
 __device__ __forceinline__ void st_global_v8(void* p, const uint32_t (&r)[8]) {
-    asm volatile("st.global.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
+    asm volatile("st.global.L1::no_allocate.v8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};"
                  :: "l"(p), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]) : "memory");
 }
 __device__ __forceinline__ void st_shared_f32(uint32_t addr, float v) {
