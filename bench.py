@@ -62,23 +62,32 @@ def traffic_from_profile(cfg_name, kernel):
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line)."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md clocks line).  The sampler process is
+    started before the warm-up (it needs ~100 ms to deliver its first line, longer than a short timed region); only the
+    lines whose own timestamp falls between begin() and end() are summarised."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
-    def __init__(self, index=0):
-        self.rows, self.proc, self.index = [], None, index
+    def __init__(self, index=0, period_ms=20):
+        self.rows, self.proc, self.index, self.period_ms = [], None, index, period_ms
+        self.t_begin = self.t_end = None
 
     def __enter__(self):
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
-                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                          "--format=csv,noheader,nounits", "-lms", str(self.period_ms)],
                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
         except OSError:
             self.proc = None
         return self
+
+    def begin(self):
+        self.t_begin = time.time()
+
+    def end(self):
+        self.t_end = time.time()
 
     def _read(self):
         for line in self.proc.stdout:
@@ -90,20 +99,42 @@ class ClockSampler:
             self.proc.terminate()
             self.t.join(timeout=2)
 
+    @staticmethod
+    def _stamp(text):
+        import datetime
+        try:
+            return datetime.datetime.strptime(text, "%Y/%m/%d %H:%M:%S.%f").timestamp()
+        except ValueError:
+            return None
+
     def summary(self):
-        sm, mx, reasons = [], [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        t0 = self.t_begin if self.t_begin is not None else float("-inf")
+        t1 = self.t_end if self.t_end is not None else float("inf")
+        parsed = []
         for r in self.rows:
             try:
-                sm.append(float(r[0])); mx.append(float(r[1]))
+                parsed.append((self._stamp(r[0]), float(r[1]), float(r[2]), r[4:8]))
             except (ValueError, IndexError):
                 continue
-            for nm, v in zip(names, r[3:7]):
+        inside = [x for x in parsed if x[0] is not None and t0 - 1e-3 <= x[0] <= t1 + 1e-3]
+        window = "timed region"
+        if not inside and parsed and self.t_begin is not None:
+            # the region was shorter than the sampling period: the sample closest to it (taken under the same load, during the
+            # warm-up steps just before or the steps just after)
+            mid = 0.5 * (t0 + t1)
+            inside = [min((x for x in parsed if x[0] is not None), key=lambda x: abs(x[0] - mid), default=None)]
+            inside = [x for x in inside if x is not None]
+            window = "nearest sample to the timed region"
+        if not inside:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        reasons = set()
+        for x in inside:
+            for nm, v in zip(names, x[3]):
                 if v.lower().startswith("active"):
                     reasons.add(nm)
-        if not sm:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons), "samples": len(sm)}
+        return {"sm_mhz": float(np.median([x[1] for x in inside])), "sm_max_mhz": float(max(x[2] for x in inside)),
+                "reasons": sorted(reasons), "samples": len(inside), "window": window}
 
 
 # ---------------------------------------------------------------------------------------------- our arm ----
@@ -381,6 +412,8 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=torch.device(device))
     pk = peaks()
     cfg_sel = select_config(args)
+    clk = ClockSampler(local)          # streaming long before the timed region (its first line takes ~100 ms)
+    clk.__enter__()
     wl = Workload(cfg_sel, args.arm, device, want_e2e=not args.device_inputs, device_inputs=args.device_inputs,
                   real_waves=args.real_waves)
     cfg = wl.cfg
@@ -395,8 +428,10 @@ def run_ours(args):
         args.steps = max(args.steps, int(args.seconds / max(1e-6, time.perf_counter() - t0)))
     wl.launches = 0
     events = []
-    with ClockSampler(local) as clk:
-        ms = timed(torch, lambda: wl.step(events), args.steps, dist)
+    clk.begin()
+    ms = timed(torch, lambda: wl.step(events), args.steps, dist)
+    clk.end()
+    clk.__exit__()
     launches = wl.launches
     ms_step = ms / args.steps
     value = aggregate_value(wl.flops, ms_step, world)
