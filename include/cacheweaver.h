@@ -70,6 +70,12 @@ typedef struct {
     int64_t actual_prefix_docs;      /* sum of the leading documents whose full 16-token blocks were all matched */
     int64_t over_predicted_docs;     /* sum of max(0, predicted - actual)                                    */
     int64_t stale_marks;             /* trie nodes marked stale (cw_mark_stale, cw_feedback, the residency-aware arm)  */
+    /* work the admitted requests ask of the device, summed over successful cw_lookup / cw_extend calls since cw_create / cw_reset
+     * (only the uncached suffix is prefilled): */
+    int64_t prompt_tokens;           /* sum of n                                                              */
+    int64_t suffix_tokens;           /* sum of n - n_cached (+ the tokens appended by cw_extend)              */
+    int64_t attn_flops;              /* sum of 4*Hq*D*[n(n+1)/2 - c(c+1)/2]: algorithmic flops of cw_prefill_attn */
+    int64_t append_bytes;            /* suffix_tokens * (2*Hq*D*2 + 4*Hkv*D*2 + 4): algorithmic bytes of cw_append_kv */
 } cw_stats_t;
 
 /* ---- lifetime ---------------------------------------------------------------------------------------- */

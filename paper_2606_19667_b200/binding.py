@@ -30,7 +30,8 @@ class CwConfig(C.Structure):
 class CwStats(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("requests", "hit_blocks", "miss_blocks", "evictions", "trie_nodes",
                                           "order_probes", "free_blocks", "seq", "predicted_prefix_docs",
-                                          "actual_prefix_docs", "over_predicted_docs", "stale_marks")]
+                                          "actual_prefix_docs", "over_predicted_docs", "stale_marks", "prompt_tokens",
+                                          "suffix_tokens", "attn_flops", "append_bytes")]
 
 
 class CwError(RuntimeError):

@@ -133,6 +133,11 @@ int cw_stats(cw_ctx* ctx, cw_stats_t* o) {
     o->actual_prefix_docs = ctx->actual_docs;
     o->over_predicted_docs = ctx->over_pred_docs;
     o->stale_marks = ctx->tree->stale_marks();
+    const cw_config& c = ctx->cfg;
+    o->prompt_tokens = ctx->blocks->prompt_tokens;
+    o->suffix_tokens = ctx->blocks->suffix_tokens;
+    o->attn_flops = 4 * (int64_t)c.num_q_heads * c.head_dim * ctx->blocks->attn_pairs;
+    o->append_bytes = ctx->blocks->suffix_tokens * (2 * (int64_t)c.num_q_heads * c.head_dim * 2 + 4 * (int64_t)c.num_kv_heads * c.head_dim * 2 + 4);
     return CW_OK;
 }
 

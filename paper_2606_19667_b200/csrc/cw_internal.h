@@ -111,6 +111,7 @@ class BlockManager {
     }
     int32_t free_list(int32_t* out, int32_t cap) const;
     int64_t requests = 0, hit_blocks = 0, miss_blocks = 0, evictions = 0;
+    int64_t prompt_tokens = 0, suffix_tokens = 0, attn_pairs = 0;   // attn_pairs: (row, key) pairs the suffixes attend to
     int32_t free_count() const { return free_count_; }
 
   private:

@@ -241,6 +241,8 @@ int BlockManager::lookup(const int32_t* tokens, int32_t n, int64_t* req, int32_t
     *n_cached = r.m * CW_BLOCK_SIZE;
     *req = next_req_++;
     ++requests; hit_blocks += r.m; miss_blocks += nblk - r.m;
+    const int64_t c = (int64_t)r.m * CW_BLOCK_SIZE;
+    prompt_tokens += n; suffix_tokens += n - c; attn_pairs += (int64_t)n * (n + 1) / 2 - c * (c + 1) / 2;
     reqs_.emplace(*req, std::move(r));
     return CW_OK;
 }
@@ -282,6 +284,7 @@ int BlockManager::extend(int64_t req, const int32_t* tokens, int32_t n_new, int3
             n_tail = 0;
         }
     }
+    suffix_tokens += n_new; attn_pairs += n_total * (n_total + 1) / 2 - (int64_t)r.n * (r.n + 1) / 2;
     r.n = (int32_t)n_total;
     if (eager_) {
         const int32_t m_keep = r.m;

@@ -187,8 +187,15 @@ def _compare_host_trace(cfg, strategy, requests=None):
         assert (a.r, a.order, a.depth, a.n_cached, a.wave) == (b.r, b.order, b.depth, b.n_cached, b.wave)
         assert a.table.tolist() == b.table
         assert np.array_equal(a.tokens, b.tokens)
-    assert runner.ctx.cw_stats()["evictions"] == ref.evictions
+    st = runner.ctx.cw_stats()
+    assert st["evictions"] == ref.evictions
     assert len(runner.waves) == ref.waves
+    # work counters of cw_stats against the plain definitions over the oracle's records
+    n = cfg.n
+    assert st["prompt_tokens"] == n * len(ref.requests)
+    assert st["suffix_tokens"] == sum(n - b.n_cached for b in ref.requests)
+    assert st["attn_flops"] == sum(4 * cfg.Hq * cfg.D * sum(p + 1 for p in range(b.n_cached, n)) for b in ref.requests)
+    assert st["append_bytes"] == st["suffix_tokens"] * (2 * cfg.Hq * cfg.D * 2 + 2 * 2 * cfg.Hkv * cfg.D * 2 + 4)
     return recs
 
 
