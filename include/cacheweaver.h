@@ -240,6 +240,35 @@ int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out,
                     const int32_t* d_block_tables, int32_t max_blocks_per_req, int32_t B, int32_t T,
                     int32_t max_q_len, int32_t max_kv_len, int32_t* d_work, void* stream);
 
+/* cw_prefill_attn_static — cw_prefill_attn for callers that cannot hand over the d_work scratch because they cannot
+ * allocate device memory: code that runs inside somebody else's process and is given only the tensors of the operation (an
+ * inference server's custom-op slot, a plugin), code inside a region where touching the allocator is forbidden (after the
+ * warm-up of a latency-critical serving loop, inside someone else's memory-pool lock), or a plain C caller that links no
+ * allocator at all.  The work list lives in a fixed array of CW_STATIC_WORK_INTS ints (2 MiB) that is part of the library
+ * image: every GPU the process uses through this library holds those 2 MiB from the moment the library's CUDA module is
+ * loaded there until the process exits.  The call itself allocates and frees nothing (no cudaMalloc / cudaFree, no library
+ * routine that allocates).
+ *   Arguments as for cw_prefill_attn, without d_work.  d_status: DEVICE int32[4], caller-owned OUTPUT, may be NULL; after
+ *   the stream has run the call it holds the first four ints of the work header (see cw_prefill_attn: [1] error flags,
+ *   [2] exact-path fallbacks, [3] number of work items).
+ *   Limit: cw_attn_work_ints(ctx, B, T) <= CW_STATIC_WORK_INTS, i.e. (T / (2*(128/g)) + B) * Hkv <= 65535 work items with
+ *   g = Hq/Hkv (config 2 of BASELINE.json needs about 10 k; a 64-request wave of the 8B shape fits up to ~520 k suffix tokens).  A
+ *   larger batch is rejected with CW_ERR_INVALID ("... exceeds the static work list ...") before anything is launched;
+ *   split the wave or use cw_prefill_attn.
+ *   Set-up: the first call on a device looks up the array's device address (cudaGetSymbolAddress) and keeps it; the
+ *   context's device (cfg.device) must be the current device of the calling thread, else CW_ERR_CUDA.  Make that first call
+ *   per device before any stream capture begins.
+ *   Sharing: there is ONE array per device, shared by every context and every call, and it keeps what the last call left
+ *   in it.  Each call rewrites all it reads (the schedule kernel resets the claim counter and the statistics and writes
+ *   the item count before the attention kernel starts), so consecutive calls on one stream are safe.  Two calls that can
+ *   run on the GPU at the same time (different streams without an event between them, two host threads) race on the
+ *   array and produce garbage: order them, or give all but one of them a d_work of their own through cw_prefill_attn. */
+#define CW_STATIC_WORK_INTS (8 * 65536)
+int cw_prefill_attn_static(cw_ctx* ctx, const void* q_roped, void* out,
+                           const int32_t* d_cu_seqlens_q, const int32_t* d_n_cached, const int32_t* d_kv_len,
+                           const int32_t* d_block_tables, int32_t max_blocks_per_req, int32_t B, int32_t T,
+                           int32_t max_q_len, int32_t max_kv_len, int32_t* d_status, void* stream);
+
 /* cw_prefill_requests — steps a7 + a8 for a wave of admitted requests in ONE call: the descriptors (cu_seqlens_q,
  * n_cached, block tables) are taken from the request handles reqs[0..B-1] (HOST, as returned by cw_lookup /
  * cw_admit_batch, in batch order; a request's rows are its tokens not yet written to the pool: the uncached suffix after

@@ -15,6 +15,7 @@ LIB_PATH = os.path.join(_PKG, "libcacheweaver.so")
 
 CW_OK, CW_ERR_INVALID, CW_ERR_NO_SPACE, CW_ERR_BAD_HANDLE, CW_ERR_CUDA = 0, -1, -2, -3, -4
 BLOCK_SIZE = 16
+STATIC_WORK_INTS = 8 * 65536          # CW_STATIC_WORK_INTS (cacheweaver.h): capacity of cw_prefill_attn_static
 ARMS = {"retrieval": 0, "greedy": 1, "sorted": 2, "recency": 3, "exhaustive": 4,      # CW_ARM_* (cacheweaver.h)
         "greedy_feedback": 5, "greedy_resident": 6}
 
@@ -88,6 +89,7 @@ def load_library(build_if_missing: bool = True):
         "cw_append_kv": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp]),
         "cw_attn_work_ints": (i64, [vp, i32, i32]),
         "cw_prefill_attn": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]),
+        "cw_prefill_attn_static": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]),
         "cw_prefill_requests_ws_bytes": (i64, [vp, i32, i32, i32]),
         "cw_prefill_requests_work_offset": (i64, [vp, i32, i32]),
         "cw_prefill_requests": (C.c_int, [vp, p(i64), i32, vp, vp, vp, vp, vp, i32, i32, vp, vp]),
@@ -105,7 +107,7 @@ def load_library(build_if_missing: bool = True):
 EXPORTS = ["cw_create", "cw_destroy", "cw_strerror", "cw_last_error", "cw_stats", "cw_pool_bytes", "cw_pool_offset", "cw_q_roped_offset",
            "cw_order", "cw_predict", "cw_order_arm", "cw_observe", "cw_mark_stale", "cw_feedback", "cw_hash_chain", "cw_lookup", "cw_release", "cw_extend", "cw_free_list",
            "cw_reset", "cw_admit_batch", "cw_release_batch",
-           "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_prefill_requests_ws_bytes",
+           "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_prefill_attn_static", "cw_prefill_requests_ws_bytes",
            "cw_prefill_requests_work_offset", "cw_prefill_requests", "cw_gather_kv", "cw_prefill_host_ws_bytes",
            "cw_prefill_host"]
 
@@ -312,6 +314,17 @@ class Context:
                                              d_kv_len.data_ptr() if d_kv_len is not None else None, d_tables.data_ptr(),
                                              max_blocks, B, T, int(max_q_len), int(max_kv_len), d_work.data_ptr(),
                                              self._stream()))
+
+    def cw_prefill_attn_static(self, q_roped, out, d_cu, d_nc, d_tables, max_blocks, B, T, max_q_len, max_kv_len,
+                               d_status=None, d_kv_len=None):
+        """cw_prefill_attn without a d_work argument, for callers that may not allocate device memory: the work list sits
+        in a 2 MiB array inside the library (one per GPU, shared by all calls: do not let two calls overlap on the GPU).
+        Raises CwError(CW_ERR_INVALID) when cw_attn_work_ints(B, T) > STATIC_WORK_INTS.  d_status: optional device int32[4]
+        that receives the work header (error flags at [1])."""
+        self._check(self.lib.cw_prefill_attn_static(
+            self.h, q_roped.data_ptr(), out.data_ptr(), d_cu.data_ptr(), d_nc.data_ptr(),
+            d_kv_len.data_ptr() if d_kv_len is not None else None, d_tables.data_ptr(), max_blocks, B, T, int(max_q_len),
+            int(max_kv_len), d_status.data_ptr() if d_status is not None else None, self._stream()))
 
     def cw_prefill_requests_ws_bytes(self, B, T, max_blocks):
         return int(self.lib.cw_prefill_requests_ws_bytes(self.h, B, T, max_blocks))

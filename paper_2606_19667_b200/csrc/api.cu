@@ -419,6 +419,29 @@ int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out, const int32_t* 
     return le ? cuda_fail(ctx, le, "cw_prefill_attn") : CW_OK;
 }
 
+// cw_prefill_attn with the work list in the library's static device array: for callers that cannot allocate device memory
+// (cacheweaver.h).  Nothing here or below allocates; a batch that needs more than CW_STATIC_WORK_INTS ints is refused.
+int cw_prefill_attn_static(cw_ctx* ctx, const void* q_roped, void* out, const int32_t* d_cu, const int32_t* d_nc,
+                           const int32_t* d_kv_len, const int32_t* d_tables, int32_t max_blocks, int32_t B, int32_t T,
+                           int32_t max_q_len, int32_t max_kv_len, int32_t* d_status, void* stream) {
+    if (!ctx || ctx->host_only) return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn_static: host-only context");
+    if (B < 0 || T < 0 || max_blocks <= 0 || max_q_len < 0 || max_kv_len < 0)
+        return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn_static: bad sizes");
+    if (cw::attn_work_ints(ctx->cfg, B, T) > (int64_t)CW_STATIC_WORK_INTS)
+        return fail(ctx, CW_ERR_INVALID,
+                    "cw_prefill_attn_static: the batch exceeds the static work list (cw_attn_work_ints(B, T) > "
+                    "CW_STATIC_WORK_INTS = 524288): split the wave or pass your own scratch to cw_prefill_attn");
+    if (T == 0 || B == 0) return CW_OK;
+    if (!q_roped || !out || !d_cu || !d_nc || !d_tables)
+        return fail(ctx, CW_ERR_INVALID, "cw_prefill_attn_static: null pointer");
+    if (max_q_len > T || (int64_t)max_kv_len > (int64_t)max_blocks * CW_BLOCK_SIZE || max_kv_len > ctx->cfg.max_position)
+        return fail(ctx, CW_ERR_INVALID,
+                    "cw_prefill_attn_static: max_q_len / max_kv_len exceed T, the block table or max_position");
+    int le = cw::launch_prefill_attn_static(ctx->cfg, q_roped, out, d_cu, d_nc, d_kv_len, d_tables, max_blocks, B, T,
+                                            max_q_len, max_kv_len, d_status, ctx->num_sms, stream);
+    return le ? cuda_fail(ctx, le, "cw_prefill_attn_static") : CW_OK;
+}
+
 // ---- one call per wave: descriptors from the request handles, one staged H2D copy, three launches ----------
 namespace {
 struct ReqWsLayout {

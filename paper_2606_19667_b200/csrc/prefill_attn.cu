@@ -35,6 +35,14 @@
 #include "cw_internal.h"
 #include "ptx_sm100.cuh"
 
+// Scratch of cw_prefill_attn_static (end of this file): the work list in memory that ships with the library.
+// Some callers have nowhere to take the d_work scratch from: a plugin running inside a host application that owns all
+// device memory and hands out only the tensors of the op, a caller inside a region where the allocator must not be
+// touched (a serving loop that forbids allocation after warm-up), a C caller without any allocator of its own.  For them
+// the item list lives in this fixed array.  It is part of the loaded module, so every GPU on which the library creates a
+// CUDA context carries its 2 MiB until the process ends; nothing is ever allocated or freed for it.
+static __device__ __align__(256) int32_t g_static_work[CW_STATIC_WORK_INTS];
+
 namespace cw {
 
 namespace {
@@ -782,6 +790,41 @@ int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, co
     if (cfg.head_dim == 128) CW_LAUNCH_ATTN(128); else CW_LAUNCH_ATTN(64);
 #undef CW_LAUNCH_ATTN
     return (int)cudaGetLastError();
+}
+
+// ---- cw_prefill_attn_static: the same two kernels with the work list in g_static_work (top of this file) ----
+namespace {
+constexpr int kMaxDevices = 64;
+// Device address of g_static_work per device ordinal.  `g_static_work` in HOST code is only a handle for the runtime's
+// symbol table, not an address a kernel may use: the address is asked for with cudaGetSymbolAddress while that device is
+// current, once per device.  A benign race between two host threads resolves the same value twice.
+int32_t* g_static_work_ptr[kMaxDevices] = {};
+}  // namespace
+
+int launch_prefill_attn_static(const cw_config& cfg, const void* q_roped, void* out, const int32_t* d_cu,
+                               const int32_t* d_nc, const int32_t* d_kv_len, const int32_t* tables, int32_t max_blocks,
+                               int32_t B, int32_t T, int32_t max_q_len, int32_t max_kv_len, int32_t* d_status, int num_sms,
+                               void* stream) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return (int)e;
+    if (dev != cfg.device || dev < 0 || dev >= kMaxDevices) return (int)cudaErrorInvalidDevice;
+    int32_t* work = g_static_work_ptr[dev];
+    if (!work) {                                        // set-up: first call on this device
+        e = cudaGetSymbolAddress((void**)&work, g_static_work);
+        if (e != cudaSuccess) return (int)e;
+        g_static_work_ptr[dev] = work;
+    }
+    // Nothing in the array has to be cleared from the host: the schedule kernel rewrites the whole header (claim counter
+    // and fallback counter to zero, error flags, item count) and every item below the count it writes; items above it
+    // are leftovers of earlier calls and are never read.
+    int le = launch_prefill_attn(cfg, q_roped, out, d_cu, d_nc, d_kv_len, tables, max_blocks, B, T, max_q_len, max_kv_len,
+                                 work, num_sms, stream);
+    if (le) return le;
+    if (d_status && attn_max_items(cfg, B, T) > 0)      // header -> caller's 4 ints, behind the attention kernel on the stream
+        return (int)cudaMemcpyAsync(d_status, work, 4 * sizeof(int32_t), cudaMemcpyDeviceToDevice,
+                                    static_cast<cudaStream_t>(stream));
+    return 0;
 }
 
 }  // namespace cw
