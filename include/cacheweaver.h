@@ -50,9 +50,11 @@ typedef struct {
                                 may be NULL together with k_pool/v_pool for a host-only context (no kernels) */
     int32_t device;          /* CUDA device ordinal (ignored for a host-only context)                       */
     int32_t index_key_bits;  /* 0 or >= 64: the prefix index is keyed by the whole 64-bit chain hash; 1..63: by its low bits only.
-                                Every index entry is also checked against a second, secretly salted 64-bit chain, so a key
-                                collision (accidental or crafted) never serves another prompt's KV: the colliding block is just
-                                not cached.  Small values make collisions frequent (used by the tests of that property).     */
+                                Every index entry is also checked against a second 64-bit chain salted with a per-context random
+                                secret, so serving another prompt's KV takes a simultaneous collision of two independent 64-bit
+                                hashes, one of them secretly salted (a colliding block is simply not cached).  This is a
+                                probabilistic safeguard built from non-cryptographic mixing, not a proof against an adversary who
+                                can observe hits.  Small values make key collisions frequent (used by the tests of that property). */
 } cw_config;
 
 typedef struct {
@@ -273,7 +275,11 @@ int cw_prefill_attn_static(cw_ctx* ctx, const void* q_roped, void* out,
  * n_cached, block tables) are taken from the request handles reqs[0..B-1] (HOST, as returned by cw_lookup /
  * cw_admit_batch, in batch order; a request's rows are its tokens not yet written to the pool: the uncached suffix after
  * cw_lookup, the appended tokens after cw_extend — prefill suffixes, prefill chunks and decode rows can share a call), written to a library-owned pinned staging slot, copied to d_ws with one
- * asynchronous H2D copy, and cw_append_kv + cw_prefill_attn are enqueued on `stream`.  Nothing is synchronised.
+ * asynchronous H2D copy, and cw_append_kv + cw_prefill_attn are enqueued on `stream`.  The call does not wait for the
+ * device, with one bound: the staging ring has 4 slots, so a call blocks on the host until the descriptor copy of the
+ * fourth-last call has completed (only a caller that runs more than four waves ahead of the GPU ever waits).
+ *   The handles advance (their rows count as written) only when the copy and both kernels were enqueued successfully: after
+ *   any error the same call can be repeated.  A handle listed twice -> CW_ERR_INVALID.
  *   q [T,Hq,D], k, v [T,Hkv,D], q_roped, out: device bf16 as in cw_append_kv / cw_prefill_attn; T must equal the sum
  *   of the requests' suffix lengths.  max_blocks_per_req >= the largest block-table length of the wave.
  *   d_ws: device scratch of cw_prefill_requests_ws_bytes() bytes, caller-owned (descriptors at offset 0: cu [B+1],

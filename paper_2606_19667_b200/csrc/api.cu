@@ -503,9 +503,13 @@ int cw_prefill_requests(cw_ctx* ctx, const int64_t* reqs, int32_t B, const void*
     int32_t* tables = reinterpret_cast<int32_t*>(static_cast<char*>(st.host) + w.tables);
     cu[0] = 0;
     int32_t max_q = 0, max_kv = 0;
+    std::unordered_set<int64_t> seen;
+    seen.reserve((size_t)B * 2);
     for (int32_t r = 0; r < B; ++r) {
         const cw::Request* rq = ctx->blocks->find(reqs[r]);
         if (!rq) return fail(ctx, CW_ERR_BAD_HANDLE, "cw_prefill_requests: unknown request handle");
+        if (!seen.insert(reqs[r]).second)       // its rows would be counted (and written) twice
+            return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: a request handle is listed twice");
         const int32_t nblk = (int32_t)rq->table.size(), c = rq->n_done, s = rq->n - c;
         if (nblk > max_blocks) return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: max_blocks too small for a request");
         if (rq->n > ctx->cfg.max_position) return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: prompt longer than max_position");
@@ -517,10 +521,6 @@ int cw_prefill_requests(cw_ctx* ctx, const int64_t* reqs, int32_t B, const void*
         max_kv = std::max(max_kv, rq->n);
     }
     if (cu[B] != T) return fail(ctx, CW_ERR_INVALID, "cw_prefill_requests: T does not match the requests' pending tokens");
-    for (int32_t r = 0; r < B; ++r) {          // everything up to n is now (being) written: the next call starts there
-        cw::Request* rq = ctx->blocks->find_mut(reqs[r]);
-        rq->n_done = rq->n;
-    }
     auto s = static_cast<cudaStream_t>(stream);
     char* ws = static_cast<char*>(d_ws);
     e = cudaMemcpyAsync(ws, st.host, desc_bytes, cudaMemcpyHostToDevice, s);
@@ -531,8 +531,14 @@ int cw_prefill_requests(cw_ctx* ctx, const int64_t* reqs, int32_t B, const void*
     const int32_t* d_tables = reinterpret_cast<const int32_t*>(ws + w.tables);
     int rc = cw_append_kv(ctx, q, k, v, q_roped, d_cu, d_nc, d_tables, max_blocks, B, T, stream);
     if (rc != CW_OK) return rc;
-    return cw_prefill_attn(ctx, q_roped, out, d_cu, d_nc, nullptr, d_tables, max_blocks, B, T, max_q, max_kv,
-                           reinterpret_cast<int32_t*>(ws + w.work), stream);
+    rc = cw_prefill_attn(ctx, q_roped, out, d_cu, d_nc, nullptr, d_tables, max_blocks, B, T, max_q, max_kv,
+                         reinterpret_cast<int32_t*>(ws + w.work), stream);
+    if (rc != CW_OK) return rc;
+    // Only now, with the copy and both kernels enqueued, do the handles move on: everything up to n is (being) written and
+    // the next call starts there.  After a failure above they are unchanged, so the same call can be repeated (writing a
+    // row's K/V twice is harmless).
+    for (int32_t r = 0; r < B; ++r) ctx->blocks->find_mut(reqs[r])->n_done = ctx->blocks->find(reqs[r])->n;
+    return CW_OK;
 }
 
 // ---- host-buffer entry point ------------------------------------------------------------------------------

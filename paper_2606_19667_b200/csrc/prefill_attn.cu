@@ -30,6 +30,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
 #include <type_traits>
 
 #include "cw_internal.h"
@@ -52,6 +53,7 @@ constexpr int kChunk = 64;           // keys per KV chunk (4 pool blocks)
 constexpr int kThreads = 512;
 constexpr int kRegsSoftmax = 136, kRegsOther = 120;   // 256 threads each: 256 * (136 + 120) = 65536 registers
 constexpr int kWorkInts = 8;         // ints per work item
+constexpr int kMaxDevices = 64;      // device ordinals with per-device launcher state (attribute flags, static work list)
 constexpr float kRescaleThreshold = 8.0f;   // log2 units
 constexpr float kSpecLimit = 65536.f;       // bound on a row sum taken against a stale reference maximum
 
@@ -773,14 +775,19 @@ int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, co
     if (e != cudaSuccess) return (int)e;
     const float scale_log2 = 1.4426950408889634f / sqrtf((float)cfg.head_dim);
     const unsigned grid = (unsigned)std::min<int64_t>(max_items, num_sms);
+    // The dynamic shared memory opt-in is a per-device attribute of the kernel: one flag per device ordinal (a process may
+    // hold contexts on several GPUs).  Two host threads racing on a flag both set the attribute, which is harmless.
+    int dev = 0;
+    e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return (int)e;
 #define CW_LAUNCH_ATTN(DD)                                                                                          \
     do {                                                                                                            \
-        static bool attr_set = false;                                                                               \
-        if (!attr_set) {                                                                                            \
+        static std::atomic<bool> attr_set[kMaxDevices];                                                             \
+        if (dev < 0 || dev >= kMaxDevices || !attr_set[dev].load(std::memory_order_acquire)) {                      \
             e = cudaFuncSetAttribute(prefill_attn_kernel<DD>, cudaFuncAttributeMaxDynamicSharedMemorySize,          \
                                      Smem<DD>::kTotal);                                                             \
             if (e != cudaSuccess) return (int)e;                                                                    \
-            attr_set = true;                                                                                        \
+            if (dev >= 0 && dev < kMaxDevices) attr_set[dev].store(true, std::memory_order_release);                \
         }                                                                                                           \
         prefill_attn_kernel<DD><<<grid, kThreads, Smem<DD>::kTotal, s>>>(                                           \
             (const __nv_bfloat16*)q_roped, (__nv_bfloat16*)out, (const __nv_bfloat16*)cfg.k_pool,                   \
@@ -794,7 +801,6 @@ int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, co
 
 // ---- cw_prefill_attn_static: the same two kernels with the work list in g_static_work (top of this file) ----
 namespace {
-constexpr int kMaxDevices = 64;
 // Device address of g_static_work per device ordinal.  `g_static_work` in HOST code is only a handle for the runtime's
 // symbol table, not an address a kernel may use: the address is asked for with cudaGetSymbolAddress while that device is
 // current, once per device.  A benign race between two host threads resolves the same value twice.

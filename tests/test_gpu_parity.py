@@ -528,3 +528,40 @@ def test_prefill_requests_equals_separate_calls(dev):
         outs[mode] = [rec.out.copy() for rec in recs]
     for a, bb in zip(outs["separate"], outs["requests"]):
         assert np.array_equal(a, bb)
+
+
+def test_prefill_requests_rejects_a_handle_listed_twice_and_leaves_the_handles_unchanged(dev):
+    """A handle listed twice would have its rows counted and written twice: CW_ERR_INVALID.  The handles only move on when the
+    copy and both launches were enqueued, so the same request can be prefilled by the next (correct) call with its full
+    suffix (n_done used to be advanced before anything was enqueued)."""
+    Hq, Hkv, D, n = 2, 1, 64, 40
+    ctx = Context(8, Hq, Hkv, D, 4, rope_theta=5e5, max_position=64, device=dev)
+    req, table, n_cached = ctx.cw_lookup(np.arange(n, dtype=np.int32))
+    assert n_cached == 0
+    rng = np.random.default_rng(5)
+    q2, k2, v2 = to_dev(rand_bits(rng, 2 * n, Hq, D), dev), to_dev(rand_bits(rng, 2 * n, Hkv, D), dev), to_dev(rand_bits(rng, 2 * n, Hkv, D), dev)
+    ws = torch.empty(ctx.cw_prefill_requests_ws_bytes(2, 2 * n, 3), dtype=torch.uint8, device=dev)
+    with pytest.raises(CwError) as e:
+        ctx.cw_prefill_requests([req, req], q2, k2, v2, torch.empty_like(q2), torch.empty_like(q2), 2 * n, 3, ws)
+    assert e.value.code == -1 and "twice" in str(e.value)
+    # the handle still has all n rows pending: T = n is accepted (T = 0 would be what a moved-on handle asks for)
+    q, k, v = q2[:n].contiguous(), k2[:n].contiguous(), v2[:n].contiguous()
+    out = torch.full_like(q, float("nan"))
+    ctx.cw_prefill_requests([req], q, k, v, torch.empty_like(q), out, n, 3, ws)
+    torch.cuda.synchronize()
+    assert torch.isfinite(out.float()).all()
+    # now the rows are written: a second call has nothing pending and T = n no longer matches
+    with pytest.raises(CwError):
+        ctx.cw_prefill_requests([req], q, k, v, torch.empty_like(q), out, n, 3, ws)
+
+
+def test_contexts_on_two_devices_both_get_the_shared_memory_opt_in():
+    """The dynamic shared memory opt-in of the attention kernel is per device: a second context on another
+    GPU must launch as well.  Needs two visible GPUs."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two visible GPUs")
+    for d in (0, 1):
+        with torch.cuda.device(d):
+            b = Batch(f"cuda:{d}", 32, 8, 128, cs=[16], ss=[70], seed=20 + d)
+            _, out, cu = b.run()
+            assert_close_attn(out[cu[0]:cu[1]], b.oracle(0), f"device {d}")
