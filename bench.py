@@ -715,7 +715,7 @@ def run_layouts(args):
             print(json.dumps({"layout": lname, "arm": arm, "requests": len(recs), "prompt_tokens_mean": float(ns.mean()),
                               "hit_blocks": int(nc.sum()) // 16, "suffix_tokens": int((ns - nc).sum()), "attn_flops": flops,
                               "predicted_docs": int(sum(rec.depth for rec in recs)),
-                              "matched_docs": int(sum(tracegen.docs_within(trace, rec.order, rec.n_cached) for rec in recs)),
+                              "matched_docs": int(sum(run.ctx.cw_matched_docs(tracegen.doc_segment_ends(trace, rec.order), rec.n_cached, len(rec.tokens)) for rec in recs)),
                               "prefill_ms": ms, "attn_tflops_incl_append": flops / ms / 1e9}), flush=True)
             del q, k, v, qr, out
 

@@ -69,7 +69,7 @@ typedef struct {
     /* predicted vs actual reusable prefix ("the trie can predict reuse for a path whose blocks were already
      * evicted"), summed over the requests admitted by cw_admit_batch and the calls of cw_feedback since cw_create/cw_reset: */
     int64_t predicted_prefix_docs;   /* sum of l(O,T)                                                        */
-    int64_t actual_prefix_docs;      /* sum of the leading documents whose full 16-token blocks were all matched */
+    int64_t actual_prefix_docs;      /* sum of the leading documents served from the cache (cw_matched_docs) */
     int64_t over_predicted_docs;     /* sum of max(0, predicted - actual)                                    */
     int64_t stale_marks;             /* trie nodes marked stale (cw_mark_stale, cw_feedback, the residency-aware arm)  */
     /* work the admitted requests ask of the device, summed over successful cw_lookup / cw_extend calls since cw_create / cw_reset
@@ -150,6 +150,18 @@ int cw_order_arm(cw_ctx* ctx, int32_t arm, const int64_t* doc_ids, int32_t k, co
  *     predicted-vs-actual counters of cw_stats.  Call it after cw_lookup and before cw_observe. */
 int cw_mark_stale(cw_ctx* ctx, const int64_t* order, int32_t k, int32_t resident_docs);
 int cw_feedback(cw_ctx* ctx, const int64_t* order, int32_t k, int32_t predicted_docs, int32_t actual_docs);
+/* The same from the engine's raw answer, so that the caller does no arithmetic of the method:
+ *   cw_matched_docs: *out_docs = number of leading documents of a prompt served from the cache, given doc_ends[k] (HOST;
+ *     doc_ends[j] = prompt position just past the segment of the j-th document: positive, non-decreasing, <= n_tokens — any
+ *     layout: headers, ragged documents), the lookup's n_cached and the prompt length n_tokens.  Reading: a
+ *     document counts when every FULL 16-token block up to its end lies inside the cached tokens (the block it shares with
+ *     the next segment cannot match on its own), measured against what cw_lookup can return at most, 16*floor((n-1)/16): a
+ *     document ending in the block of the last prompt token is not punished for the cap.  Pure.
+ *   cw_feedback_tokens = cw_matched_docs + cw_feedback(order, predicted_docs, that count); *out_actual_docs (may be NULL)
+ *     receives the count.  cw_admit_batch applies the same rule with doc_ends[j] = (j+1)*doc_len. */
+int cw_matched_docs(cw_ctx* ctx, const int32_t* doc_ends, int32_t k, int32_t n_cached, int32_t n_tokens, int32_t* out_docs);
+int cw_feedback_tokens(cw_ctx* ctx, const int64_t* order, int32_t k, int32_t predicted_docs, const int32_t* doc_ends,
+                       int32_t n_cached, int32_t n_tokens, int32_t* out_actual_docs);
 
 /* ---- prefix cache, host (PAPER.md:33 chained block hashes; PAPER.md:129 block eviction) -------------- */
 /* chain[i] = FNV1a64(LE64(chain[i-1]) || 16 x LE32(token)), chain[-1] = hash_salt, i < floor(n/16). */

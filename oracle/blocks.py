@@ -192,3 +192,22 @@ class BlockManager:
         assert len(self.index) == sum(1 for k in self.key_of if k is not None)
         for k, b in self.index.items():
             assert self.key_of[b] == k, "index <-> has_hash bijection broken"
+
+
+def matched_docs(doc_ends, n_cached: int, n_tokens: int) -> int:
+    """Leading documents of a prompt that count as served from the cache (the `actual` of the feedback rule; SURVEY.md 8(f)
+    NEXT-1, PAPER.md:129-141 "the trie predicts a long reusable prefix ... the supposed cached path is probably gone",
+    :314).  Reading: doc_ends[j] is the prompt position just past the segment of the j-th document; a document
+    counts when every FULL 16-token block up to its end was matched — the block it shares with what follows cannot match
+    unless the next segment matches too — and "matched" is measured against what a lookup can ever return: it never
+    matches the block that holds the last prompt token (c3: m <= floor((n-1)/16)), so a document that ends in that block is
+    not punished for it (a prompt of block-aligned documents and no query would otherwise lose its last document every
+    time).  Plain count, no state.  Pins: tests/test_oracle_residency.py (hand-worked ragged segment ends; the
+    no-query case)."""
+    cap = (n_tokens - 1) // BS * BS
+    m = 0
+    for end in doc_ends:
+        if min(end // BS * BS, cap) > n_cached:
+            break
+        m += 1
+    return m

@@ -18,7 +18,7 @@ import numpy as np
 
 import tracegen
 from .attention import PagedPool, attention_suffix, attention_full
-from .blocks import BlockManager, NoSpace, chain_hashes
+from .blocks import BlockManager, NoSpace, chain_hashes, matched_docs
 from .ordering import KnowledgeTree
 from .strategies import RecencyOrder, order_exhaustive, order_sorted
 
@@ -108,7 +108,7 @@ def run_trace(trace, strategy: str = "greedy", compute: bool = True, requests=No
             close_wave()
             continue                        # retry the same request in the next wave (order() is pure)
         if strategy in ("greedy_feedback", "greedy_resident"):
-            tree.feedback(O, depth, tracegen.docs_within(trace, O, c))
+            tree.feedback(O, depth, matched_docs(tracegen.doc_segment_ends(trace, O), c, len(tokens)))
         tree.observe(O)
         recency.observe(O)
         rr = RequestResult(r, O, depth, tokens, table, c, wave)

@@ -77,6 +77,8 @@ def load_library(build_if_missing: bool = True):
         "cw_observe": (C.c_int, [vp, p(i64), i32]),
         "cw_mark_stale": (C.c_int, [vp, p(i64), i32, i32]),
         "cw_feedback": (C.c_int, [vp, p(i64), i32, i32, i32]),
+        "cw_matched_docs": (C.c_int, [vp, p(i32), i32, i32, i32, p(i32)]),
+        "cw_feedback_tokens": (C.c_int, [vp, p(i64), i32, i32, p(i32), i32, i32, p(i32)]),
         "cw_hash_chain": (C.c_int, [vp, p(i32), i32, p(C.c_uint64)]),
         "cw_lookup": (C.c_int, [vp, p(i32), i32, i32, p(i64), p(i32), p(i32)]),
         "cw_release": (C.c_int, [vp, i64]),
@@ -105,7 +107,7 @@ def load_library(build_if_missing: bool = True):
 
 
 EXPORTS = ["cw_create", "cw_destroy", "cw_strerror", "cw_last_error", "cw_stats", "cw_pool_bytes", "cw_pool_offset", "cw_q_roped_offset",
-           "cw_order", "cw_predict", "cw_order_arm", "cw_observe", "cw_mark_stale", "cw_feedback", "cw_hash_chain", "cw_lookup", "cw_release", "cw_extend", "cw_free_list",
+           "cw_order", "cw_predict", "cw_order_arm", "cw_observe", "cw_mark_stale", "cw_feedback", "cw_matched_docs", "cw_feedback_tokens", "cw_hash_chain", "cw_lookup", "cw_release", "cw_extend", "cw_free_list",
            "cw_reset", "cw_admit_batch", "cw_release_batch",
            "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_prefill_attn_static", "cw_prefill_requests_ws_bytes",
            "cw_prefill_requests_work_offset", "cw_prefill_requests", "cw_gather_kv", "cw_prefill_host_ws_bytes",
@@ -214,6 +216,20 @@ class Context:
     def cw_feedback(self, order, predicted_docs, actual_docs):
         d = np.ascontiguousarray(order, dtype=np.int64)
         self._check(self.lib.cw_feedback(self.h, _i64p(d), len(d), int(predicted_docs), int(actual_docs)))
+
+    def cw_matched_docs(self, doc_ends, n_cached, n_tokens):
+        e = _np_i32(doc_ends)
+        out = C.c_int32()
+        self._check(self.lib.cw_matched_docs(self.h, _i32p(e), len(e), int(n_cached), int(n_tokens), C.byref(out)))
+        return out.value
+
+    def cw_feedback_tokens(self, order, predicted_docs, doc_ends, n_cached, n_tokens):
+        """cw_feedback with the matched-document count taken by the library from the lookup's n_cached; returns the count."""
+        d, e = np.ascontiguousarray(order, dtype=np.int64), _np_i32(doc_ends)
+        out = C.c_int32()
+        self._check(self.lib.cw_feedback_tokens(self.h, _i64p(d), len(d), int(predicted_docs), _i32p(e), int(n_cached),
+                                                int(n_tokens), C.byref(out)))
+        return out.value
 
     # ---- prefix cache ----
     def cw_hash_chain(self, tokens):

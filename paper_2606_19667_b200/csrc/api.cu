@@ -26,6 +26,20 @@ bool bad_cfg(const cw_config* c) {
            c->num_q_heads / c->num_kv_heads > 128;
 }
 inline int64_t align256(int64_t x) { return (x + 255) / 256 * 256; }
+// Leading documents served from the cache (cacheweaver.h: cw_matched_docs).  end(j) = prompt position just past document j.
+template <class EndFn>
+int32_t count_matched_docs(EndFn end, int32_t k, int64_t n_cached, int64_t n_tokens) {
+    const int64_t cap = (n_tokens - 1) / CW_BLOCK_SIZE * CW_BLOCK_SIZE;   // a lookup never matches the last token's block
+    int32_t m = 0;
+    while (m < k && std::min<int64_t>((int64_t)end(m) / CW_BLOCK_SIZE * CW_BLOCK_SIZE, cap) <= n_cached) ++m;
+    return m;
+}
+bool bad_doc_ends(const int32_t* ends, int32_t k, int32_t n_cached, int32_t n_tokens) {
+    if (k < 0 || (k > 0 && !ends) || n_tokens <= 0 || n_cached < 0 || n_cached > n_tokens) return true;
+    for (int32_t j = 0; j < k; ++j)
+        if (ends[j] <= 0 || ends[j] > n_tokens || (j > 0 && ends[j] < ends[j - 1])) return true;
+    return false;
+}
 
 }  // namespace
 
@@ -191,6 +205,24 @@ int cw_feedback(cw_ctx* ctx, const int64_t* order, int32_t k, int32_t predicted_
     return CW_OK;
 }
 
+int cw_matched_docs(cw_ctx* ctx, const int32_t* doc_ends, int32_t k, int32_t n_cached, int32_t n_tokens, int32_t* out_docs) {
+    if (!ctx || !out_docs || bad_doc_ends(doc_ends, k, n_cached, n_tokens))
+        return fail(ctx, CW_ERR_INVALID, "cw_matched_docs: bad argument (doc_ends must be positive, non-decreasing, <= n_tokens)");
+    *out_docs = count_matched_docs([&](int32_t j) { return doc_ends[j]; }, k, n_cached, n_tokens);
+    return CW_OK;
+}
+
+int cw_feedback_tokens(cw_ctx* ctx, const int64_t* order, int32_t k, int32_t predicted_docs, const int32_t* doc_ends,
+                       int32_t n_cached, int32_t n_tokens, int32_t* out_actual_docs) {
+    int32_t actual = 0;
+    if (!ctx || (k > 0 && !order) || predicted_docs < 0 || predicted_docs > k)
+        return fail(ctx, CW_ERR_INVALID, "cw_feedback_tokens: bad argument");
+    const int rc = cw_matched_docs(ctx, doc_ends, k, n_cached, n_tokens, &actual);
+    if (rc != CW_OK) return rc;
+    if (out_actual_docs) *out_actual_docs = actual;
+    return cw_feedback(ctx, order, k, predicted_docs, actual);
+}
+
 int cw_order_arm(cw_ctx* ctx, int32_t arm, const int64_t* doc_ids, int32_t k, const int32_t* doc_tokens, int32_t num_docs,
                  int32_t doc_len, const int32_t* query_tokens, int32_t q_len, int64_t* out_order, int32_t* out_pred) {
     if (!ctx || k < 0 || (k > 0 && (!doc_ids || !out_order)) || arm < CW_ARM_RETRIEVAL || arm > CW_ARM_GREEDY_RESIDENT)
@@ -344,8 +376,7 @@ int cw_admit_batch(cw_ctx* ctx, const int64_t* doc_ids, int32_t B, int32_t k, in
         if (rc != CW_OK) return rc;
         for (int32_t i = nblk; i < max_blocks; ++i) table[i] = 0;
         {   // predicted vs actual prefix: documents all of whose full 16-token blocks are inside the cached tokens
-            int32_t actual = 0;
-            while (actual < k && (int64_t)(actual + 1) * doc_len / CW_BLOCK_SIZE * CW_BLOCK_SIZE <= out_nc[r]) ++actual;
+            const int32_t actual = count_matched_docs([&](int32_t j) { return (int64_t)(j + 1) * doc_len; }, k, out_nc[r], n);
             if (reorder == CW_ARM_GREEDY_FEEDBACK || reorder == CW_ARM_GREEDY_RESIDENT) {
                 cw_feedback(ctx, O, k, out_pred[r], actual);
             } else {

@@ -96,7 +96,7 @@ class TraceRunner:
         tokens = tracegen.assemble_prompt(self.trace, r, O)
         req, table, c = self.ctx.cw_lookup(tokens)        # raises NoSpace with state unchanged
         if self.strategy in ("greedy_feedback", "greedy_resident"):
-            self.ctx.cw_feedback(O, depth, tracegen.docs_within(self.trace, O, c))
+            self.ctx.cw_feedback_tokens(O, depth, tracegen.doc_segment_ends(self.trace, O), c, len(tokens))
         self.ctx.cw_observe(O)
         return req, RequestRecord(r, O, depth, tokens, table, c, len(self.waves))
 

@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 
 import tracegen
-from oracle.blocks import BlockManager
+from oracle.blocks import BlockManager, matched_docs
 from oracle.pipeline import run_trace
 from paper_2606_19667_b200.engine import TraceRunner
 
@@ -81,13 +81,13 @@ def test_library_matches_oracle_on_the_literal_layout(strategy):
 
 def test_feedback_does_not_punish_the_lost_partial_block():
     """With unaligned documents the block a document shares with the next header is never matched; a document counts as
-    matched when all its FULL blocks are (tracegen.docs_within), so the feedback arm marks nothing stale without eviction
+    matched when all its FULL blocks are (oracle.blocks.matched_docs), so the feedback arm marks nothing stale without eviction
     and orders exactly like plain greedy."""
     trace = tracegen.make_trace(literal_config())
     a = run_trace(trace, "greedy", compute=False)
     b = run_trace(trace, "greedy_feedback", compute=False)
     assert [r.order for r in a.requests] == [r.order for r in b.requests]
-    assert all(r.depth == tracegen.docs_within(trace, r.order, r.n_cached) for r in a.requests)
+    assert all(r.depth == matched_docs(tracegen.doc_segment_ends(trace, r.order), r.n_cached, len(r.tokens)) for r in a.requests)
 
 
 @pytest.mark.gpu

@@ -11,7 +11,7 @@ import pytest
 
 import tracegen
 from conftest import golden
-from oracle.blocks import BlockManager
+from oracle.blocks import BlockManager, matched_docs
 from oracle.ordering import KnowledgeTree
 from oracle.pipeline import run_trace
 
@@ -122,3 +122,54 @@ def test_resident_arm_predicts_exactly_and_never_beats_exhaustive(seed):
         T.feedback(O, T.ell(O), c // cfg.doc_len)
         T.observe(O)
         bm.release(req)
+
+
+def test_matched_docs_hand_worked_ragged_segments():
+    """oracle.blocks.matched_docs on a hand-worked literal-layout prompt: 30 instruction tokens, then per document a
+    7-token header, the passage and a blank-line token; passages of 200, 190 and 206 tokens, a 50-token question part:
+       doc ends 30+208 = 238, 238+198 = 436, 436+214 = 650; n = 700.
+    Full blocks up to each end: 224, 432, 640 tokens.  A lookup that returned n_cached = 224 served document 1 whole
+    (its last 14 tokens share a block with header 2 and can never match alone); 432 serves two, 640 all three; one block
+    less each time loses the document."""
+    ends, n = [238, 436, 650], 700
+    assert [matched_docs(ends, c, n) for c in (0, 208, 224, 416, 432, 624, 640, 688)] == [0, 0, 1, 1, 2, 2, 3, 3]
+    assert matched_docs([], 64, 100) == 0
+
+
+def test_matched_docs_does_not_punish_the_lookup_cap():
+    """Three block-aligned 32-token documents and NO query: n = 96, and a lookup can return at most 16*floor(95/16) = 80
+    cached tokens.  With everything resident (n_cached = 80) all three documents count (the uncapped rule
+    said 2, so the feedback arm marked a fully resident leaf stale on every repeat).  With a one-token query (n = 97) the
+    cap is 96 and the third document needs n_cached = 96."""
+    assert matched_docs([32, 64, 96], 80, 96) == 3
+    assert matched_docs([32, 64, 96], 64, 96) == 2
+    assert matched_docs([32, 64, 96], 80, 97) == 2
+    assert matched_docs([32, 64, 96], 96, 97) == 3
+
+
+def _all_nodes(tree):
+    stack, out = [tree.root], []
+    while stack:
+        node = stack.pop()
+        for c in node.children.values():
+            out.append(c)
+            stack.append(c)
+    return out
+
+
+def test_repeated_prompt_without_query_is_never_marked_stale():
+    """the same 3 documents, no query, served repeatedly through the oracle pipeline with the feedback arm: predicted ==
+    actual on every repeat and no node is ever marked stale."""
+    bm, tree = BlockManager(24), KnowledgeTree(12)
+    rng = np.random.default_rng(0)
+    docs = {d: rng.integers(0, 32000, size=32, dtype=np.int32) for d in (5, 6, 7)}
+    for rep in range(4):
+        O, depth = tree.order([7, 5, 6])
+        tokens = np.concatenate([docs[d] for d in O])
+        req, table, c = bm.lookup(tokens)
+        actual = matched_docs([32, 64, 96], c, len(tokens))
+        assert (depth, actual, c) == ((0, 0, 0) if rep == 0 else (3, 3, 80))
+        tree.feedback(O, depth, actual)
+        tree.observe(O)
+        bm.release(req)
+        assert all(node.stale_epoch == 0 for node in _all_nodes(tree))

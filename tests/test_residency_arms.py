@@ -90,3 +90,39 @@ def test_block_table_scenario_rows_through_the_c_abi():
     retr, order, depth = [x.split() for x in g["req5a_after_feedback"].split("|")]
     O, d = ctx.cw_order([ids[c] for c in retr])
     assert ([names[i] for i in O], d) == (order, int(depth[0]))
+
+
+def test_matched_docs_through_the_c_abi():
+    """cw_matched_docs on the hand-worked ragged prompt and the no-query prompt of tests/test_oracle_residency.py (expected
+    values typed here, not taken from the oracle), then against the oracle on random segment ends."""
+    from oracle.blocks import matched_docs
+    ctx = Context(16, 2, 1, 64, 8)
+    ends, n = [238, 436, 650], 700
+    assert [ctx.cw_matched_docs(ends, c, n) for c in (0, 208, 224, 416, 432, 624, 640, 688)] == [0, 0, 1, 1, 2, 2, 3, 3]
+    assert ctx.cw_matched_docs([32, 64, 96], 80, 96) == 3 and ctx.cw_matched_docs([32, 64, 96], 80, 97) == 2
+    rng = np.random.default_rng(3)
+    for _ in range(300):
+        k = int(rng.integers(0, 7))
+        ends = np.cumsum(rng.integers(1, 70, size=k)).tolist()
+        n = (ends[-1] if k else 1) + int(rng.integers(0, 40))
+        c = 16 * int(rng.integers(0, (n - 1) // 16 + 1))
+        assert ctx.cw_matched_docs(ends, c, n) == matched_docs(ends, c, n), (ends, c, n)
+    for bad in ([0, 5], [9, 4], [5, 800]):
+        with pytest.raises(Exception):
+            ctx.cw_matched_docs(bad, 0, 700)
+
+
+def test_admit_batch_without_query_counts_the_last_document():
+    """3 block-aligned documents and q_len = 0, the same request repeated.  The lookup cap (floor((n-1)/16) blocks)
+    keeps the last block out of every match; the matched-document count allows for it, so predicted == actual on every
+    repeat and the feedback arm marks nothing stale."""
+    ctx = Context(24, 2, 1, 64, 12)
+    rng = np.random.default_rng(1)
+    doc_tokens = rng.integers(0, 32000, size=(8, 32), dtype=np.int32)
+    for rep in range(4):
+        res = ctx.cw_admit_batch(np.array([[7, 5, 6]], dtype=np.int64), "greedy_feedback", doc_tokens,
+                                 np.zeros((1, 0), dtype=np.int32))
+        assert int(res["n_cached"][0]) == (0 if rep == 0 else 80)
+        ctx.cw_release_batch(res["reqs"])
+    st = ctx.cw_stats()
+    assert (st["predicted_prefix_docs"], st["actual_prefix_docs"], st["over_predicted_docs"], st["stale_marks"]) == (9, 9, 0, 0)

@@ -191,17 +191,15 @@ def doc_prefix_tokens(trace: Trace, docs) -> np.ndarray:
     return np.ascontiguousarray(np.concatenate(parts), dtype=np.int32)
 
 
-def docs_within(trace: Trace, order, n_tokens: int) -> int:
-    """number of leading documents of `order` covered by the first n_tokens prompt tokens: every FULL 16-token block up to
-    the end of the document's segment lies inside them (the block a document shares with what follows can never be
-    matched unless the next segment matches too; for block-aligned documents this is plain containment)."""
-    pos, m = 0, 0
+def doc_segment_ends(trace: Trace, order) -> list:
+    """prompt position just past the segment of each document of `order` (cumulative segment lengths: prompt structure
+    only — what counts as a matched document is decided by the oracle and by the library, each on its own)."""
+    pos, ends = 0, []
     for key, t in segments(trace, None, order):
         pos += len(t)
-        if pos // BLOCK_SIZE * BLOCK_SIZE > n_tokens:
-            break
-        m += key[0] == 0
-    return m
+        if key[0] == 0:
+            ends.append(pos)
+    return ends
 
 
 def f32_to_bf16_bits(x: np.ndarray) -> np.ndarray:
