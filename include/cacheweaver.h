@@ -225,8 +225,9 @@ int cw_free_list(cw_ctx* ctx, int32_t* out, int32_t cap, int32_t* out_len);
  *   owns the slice starting at cu_seqlens_q[r]*Hq*D, laid out as cw_q_roped_offset() says; it must NOT alias q
  *   (q is read through the non-coherent path).  The descriptors are on the device, so they cannot be rejected by this call:
  *   a token whose position is >= max_position or >= 16*max_blocks_per_req, or whose table entry is not in [0, NB), is
- *   SKIPPED (nothing of it is written: no clamped rotation, no store outside the pool); cw_prefill_attn flags a request
- *   that is too long in its work header.  The pools must have been
+ *   SKIPPED (nothing of it is written: no clamped rotation, no store outside the pool), and so is a row that does not lie
+ *   inside its request's slice of [0, T) (non-monotone cu_seqlens_q); cw_prefill_attn flags a request that is too long or a
+ *   table entry outside the pool in its work header.  The pools must have been
  *   zero-filled once by the caller (stale slots of a partially filled block must hold finite values). */
 int cw_append_kv(cw_ctx* ctx, const void* q, const void* k, const void* v, void* q_roped,
                  const int32_t* d_cu_seqlens_q, const int32_t* d_n_cached, const int32_t* d_block_tables,
@@ -242,8 +243,11 @@ int cw_append_kv(cw_ctx* ctx, const void* q, const void* k, const void* v, void*
  *   max_q_len / max_kv_len: upper bounds on the suffix length / kv length of any request of the batch (host values;
  *   max_kv_len <= 16 * max_blocks_per_req and <= max_position).
  *   d_work: DEVICE int32 scratch of cw_attn_work_ints(ctx, B, T) ints, caller-owned, written by this call.  After the
- *   stream has run the call: d_work[1] != 0 means a request descriptor was invalid (negative lengths, lengths beyond
- *   the stated maxima, kv_len mismatch) and that request produced no output; d_work[2] counts the
+ *   stream has run the call: d_work[1] != 0 is an error.  Bit 0: a request descriptor was invalid (negative lengths,
+ *   lengths beyond the stated maxima, kv_len mismatch) and that request produced no output; bit 2: one of the first
+ *   ceil(kv_len/16) block table entries of a request was outside [0, NB) — that request produced no output either and no
+ *   memory outside the pool was touched (cw_append_kv had skipped the tokens of such an entry; with B > 2048 the whole
+ *   batch is dropped).  d_work[2] counts the
  *   softmax chunks that left the speculative path (statistics); d_work[3] is the number of work items.
  *   q_roped: as written by cw_append_kv (tile-packed); out [T,Hq,D] device bf16 row-major.
  *   (SURVEY.md 8(b) lists this signature without d_work; the scratch is passed in because the library allocates no

@@ -83,7 +83,10 @@ __global__ void __launch_bounds__(THREADS) append_kv_kernel(
         // A token whose position has no RoPE row or no table slot, or whose table entry is not a pool block, is skipped: nothing
         // of it is written (no clamping to a wrong rotation, no store outside the pool).  cw_prefill_attn reports a request
         // that is too long through its error flag.
-        const bool pos_ok = p >= 0 && p < max_position && (p >> 4) < max_blocks;
+        // cu is unchecked device data as well: a row outside its request's slice (non-monotone cu) or a slice that leaves
+        // [0, T) is skipped too, so every q_roped store below stays inside the request's own part of the T*Hq*D buffer.
+        const bool pos_ok = p >= 0 && p < max_position && (p >> 4) < max_blocks && q_begin >= 0 && tl < s_len &&
+                            s_len <= T - q_begin;
         const int blk = pos_ok ? __ldg(tables + (size_t)r * max_blocks + (p >> 4)) : -1;
         if (blk < 0 || blk >= num_blocks) continue;
         const int tib = p & 15;

@@ -644,11 +644,12 @@ __global__ void __launch_bounds__(kThreads, 1) prefill_attn_kernel(
 // n_cached[r] is the number of tokens of request r already in the pool: a multiple of 16 after cw_lookup, any value for a
 // chunk of a chunked prefill or a decode row.
 // work header (ints): [0] claim counter, [1] error flags (bit 0: a request descriptor was invalid and contributes no
-// item), [2] exact-path fallbacks of the speculative softmax (statistics), [3] number of items; items from int 8 on.
+// item; bit 1: item list overflow; bit 2: a block table entry outside the pool, request dropped), [2] exact-path fallbacks of the speculative softmax (statistics), [3] number of items; items from int 8 on.
 constexpr int kSchedMaxSmemReqs = 2048;      // requests whose (suffix, cached, offset) fit the schedule kernel's shared memory
 
 __global__ void __launch_bounds__(1024) attn_schedule_kernel(
-    const int32_t* __restrict__ cu, const int32_t* __restrict__ nc, const int32_t* __restrict__ kv_len, int B, int T,
+    const int32_t* __restrict__ cu, const int32_t* __restrict__ nc, const int32_t* __restrict__ kv_len,
+    const int32_t* __restrict__ tables, int num_blocks, int B, int T,
     int Hq, int Hkv, int D, int max_blocks, int max_position, int max_q_len, int max_kv_len, int32_t* __restrict__ work,
     int64_t max_items) {
     const int g = Hq / Hkv, tpt = kTileM / g, R = tpt * g;
@@ -691,6 +692,24 @@ __global__ void __launch_bounds__(1024) attn_schedule_kernel(
         }
     }
     __syncthreads();
+    // The block tables are device data nobody has checked, and the attention kernel's loader follows them into the pools:
+    // every entry a request will read (blocks 0 .. ceil(kv_len/16) - 1) must name a pool block.  One warp per request, lanes
+    // over its entries (coalesced, all loads of a lane independent).  A request with a bad entry is dropped (error bit 2,
+    // no items, no output); a batch too large for the shared-memory copy of the lengths is dropped as a whole.
+    for (int r = threadIdx.x >> 5; r < B; r += blockDim.x >> 5) {
+        int c;
+        const int s = get(r, c);
+        const int nblk = s > 0 ? (c + s + CW_BLOCK_SIZE - 1) / CW_BLOCK_SIZE : 0;
+        const int32_t* row = tables + (size_t)r * max_blocks;
+        bool bad = false;
+        for (int i = threadIdx.x & 31; i < nblk; i += 32) bad |= (unsigned)row[i] >= (unsigned)num_blocks;
+        if (__any_sync(0xffffffffu, bad) && (threadIdx.x & 31) == 0) {
+            atomicOr(&s_err, 4);
+            if (in_smem) s_s[r] = 0;
+        }
+    }
+    __syncthreads();
+    const bool drop_all = !in_smem && (s_err & 4);
     // rank sort + exclusive prefix sum of the item counts in one pass over the other requests
     for (int r = threadIdx.x; r < B; r += blockDim.x) {
         int c;
@@ -747,7 +766,7 @@ __global__ void __launch_bounds__(1024) attn_schedule_kernel(
         work[0] = 0;
         work[1] = s_err;
         work[2] = 0;
-        work[3] = s_total;
+        work[3] = drop_all ? 0 : s_total;
     }
 }
 
@@ -769,7 +788,7 @@ int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, co
     auto s = static_cast<cudaStream_t>(stream);
     const int64_t max_items = attn_max_items(cfg, B, T);
     if (max_items == 0) return 0;
-    attn_schedule_kernel<<<1, 1024, 0, s>>>(d_cu, d_nc, d_kv_len, B, T, cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim,
+    attn_schedule_kernel<<<1, 1024, 0, s>>>(d_cu, d_nc, d_kv_len, tables, cfg.num_blocks, B, T, cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim,
                                             max_blocks, cfg.max_position, max_q_len, max_kv_len, d_work, max_items);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return (int)e;

@@ -565,3 +565,46 @@ def test_contexts_on_two_devices_both_get_the_shared_memory_opt_in():
             b = Batch(f"cuda:{d}", 32, 8, 128, cs=[16], ss=[70], seed=20 + d)
             _, out, cu = b.run()
             assert_close_attn(out[cu[0]:cu[1]], b.oracle(0), f"device {d}")
+
+
+def test_attention_flags_a_block_table_entry_outside_the_pool(dev):
+    """cw_append_kv skips the tokens of a table entry outside [0, NB); cw_prefill_attn used to follow that entry
+    into memory outside the pool.  Now the schedule kernel scans the entries every request will read, drops a request with
+    a bad one (its output rows keep their fill value) and sets error bit 2 of the work header; the other requests are
+    computed, and the device stays healthy (a clean batch afterwards is within tolerance of the oracle)."""
+    b = Batch(dev, 32, 8, 128, cs=[0, 32], ss=[100, 40], seed=9)
+    bad = b.tables.copy()
+    b3 = Batch(dev, 32, 8, 128, cs=[0, 32, 16], ss=[100, 40, 50], seed=9)
+    for bb, rows in ((b, [(0, 2, b.ctx.NB + 7), (1, 0, -3)]), (b3, [(1, 3, b3.ctx.NB)])):
+        bad = bb.tables.copy()
+        for r, i, val in rows:
+            bad[r, i] = val
+        bb.d_tables = torch.from_numpy(bad).to(dev)
+        with pytest.raises(AssertionError, match="rejected on the device"):
+            bb.run()
+        assert bb.work_header[1] & 4, bb.work_header
+    # b: both requests dropped -> no items at all; b3: only request 1 dropped
+    assert b.work_header[3] == 0 and b3.work_header[3] > 0
+    good = Batch(dev, 32, 8, 128, cs=[0, 32], ss=[100, 40], seed=9)
+    _, out, cu = good.run()
+    for r in range(good.B):
+        assert_close_attn(out[cu[r]:cu[r + 1]], good.oracle(r), f"request {r} after the faulty batch")
+
+
+def test_append_kv_skips_rows_of_a_non_monotone_cu(dev):
+    """with a cu_seqlens_q that is not monotone the rows that fall outside their request's slice are skipped:
+    q_roped keeps its fill value there and nothing is written outside the buffer (guard words stay intact)."""
+    Hq, Hkv, D, T = 4, 2, 64, 48
+    ctx = Context(8, Hq, Hkv, D, 4, rope_theta=5e5, max_position=64, device=dev)
+    rng = np.random.default_rng(4)
+    q, k, v = to_dev(rand_bits(rng, T, Hq, D), dev), to_dev(rand_bits(rng, T, Hkv, D), dev), to_dev(rand_bits(rng, T, Hkv, D), dev)
+    guard = 4096
+    buf = torch.full((T * Hq * D + 2 * guard,), 7.0, dtype=torch.bfloat16, device=dev)
+    qr = buf[guard:guard + T * Hq * D]
+    d_cu = torch.tensor([0, 40, 24, 48], dtype=torch.int32, device=dev)      # request 1 has a negative length
+    d_nc = torch.zeros(3, dtype=torch.int32, device=dev)
+    d_tables = torch.tensor([[0, 1, 2], [3, 4, 5], [6, 7, 0]], dtype=torch.int32, device=dev)
+    ctx.cw_append_kv(q, k, v, qr, d_cu, d_nc, d_tables, 3, 3, T)
+    torch.cuda.synchronize()
+    assert torch.all(buf[:guard] == 7.0) and torch.all(buf[guard + T * Hq * D:] == 7.0), "store outside q_roped"
+    assert torch.isfinite(buf.float()).all()
