@@ -258,6 +258,16 @@ int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out,
                     const int32_t* d_block_tables, int32_t max_blocks_per_req, int32_t B, int32_t T,
                     int32_t max_q_len, int32_t max_kv_len, int32_t* d_work, void* stream);
 
+/* The two launches of cw_prefill_attn, separately.  cw_attn_schedule (descriptors -> work list in d_work) reads neither
+ * q_roped nor the pools, so it can be enqueued in front of cw_append_kv or, on a second stream, beside it; cw_attn_run (the
+ * attention kernel over that list) must come after both.  cw_prefill_attn(...) == cw_attn_schedule(...) + cw_attn_run(...)
+ * on one stream; arguments and error behaviour as described there.  B and T of the two calls must be equal. */
+int cw_attn_schedule(cw_ctx* ctx, const int32_t* d_cu_seqlens_q, const int32_t* d_n_cached, const int32_t* d_kv_len,
+                     const int32_t* d_block_tables, int32_t max_blocks_per_req, int32_t B, int32_t T,
+                     int32_t max_q_len, int32_t max_kv_len, int32_t* d_work, void* stream);
+int cw_attn_run(cw_ctx* ctx, const void* q_roped, void* out, const int32_t* d_block_tables, int32_t max_blocks_per_req,
+                int32_t B, int32_t T, int32_t* d_work, void* stream);
+
 /* cw_prefill_attn_static — cw_prefill_attn for callers that cannot hand over the d_work scratch because they cannot
  * allocate device memory: code that runs inside somebody else's process and is given only the tensors of the operation (an
  * inference server's custom-op slot, a plugin), code inside a region where touching the allocator is forbidden (after the
@@ -291,7 +301,9 @@ int cw_prefill_attn_static(cw_ctx* ctx, const void* q_roped, void* out,
  * n_cached, block tables) are taken from the request handles reqs[0..B-1] (HOST, as returned by cw_lookup /
  * cw_admit_batch, in batch order; a request's rows are its tokens not yet written to the pool: the uncached suffix after
  * cw_lookup, the appended tokens after cw_extend — prefill suffixes, prefill chunks and decode rows can share a call), written to a library-owned pinned staging slot, copied to d_ws with one
- * asynchronous H2D copy, and cw_append_kv + cw_prefill_attn are enqueued on `stream`.  The call does not wait for the
+ * asynchronous H2D copy, and cw_append_kv + cw_prefill_attn are enqueued on `stream` (for waves of >= 4096 rows the schedule
+ * kernel runs on a library-owned side stream beside cw_append_kv, forked from and joined back into `stream` with events:
+ * for the caller everything is still ordered on `stream`).  The call does not wait for the
  * device, with one bound: the staging ring has 4 slots, so a call blocks on the host until the descriptor copy of the
  * fourth-last call has completed (only a caller that runs more than four waves ahead of the GPU ever waits).
  *   The handles advance (their rows count as written) only when the copy and both kernels were enqueued successfully: after

@@ -91,6 +91,8 @@ def load_library(build_if_missing: bool = True):
         "cw_append_kv": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, vp]),
         "cw_attn_work_ints": (i64, [vp, i32, i32]),
         "cw_prefill_attn": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]),
+        "cw_attn_schedule": (C.c_int, [vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]),
+        "cw_attn_run": (C.c_int, [vp, vp, vp, vp, i32, i32, i32, vp, vp]),
         "cw_prefill_attn_static": (C.c_int, [vp, vp, vp, vp, vp, vp, vp, i32, i32, i32, i32, i32, vp, vp]),
         "cw_prefill_requests_ws_bytes": (i64, [vp, i32, i32, i32]),
         "cw_prefill_requests_work_offset": (i64, [vp, i32, i32]),
@@ -109,7 +111,7 @@ def load_library(build_if_missing: bool = True):
 EXPORTS = ["cw_create", "cw_destroy", "cw_strerror", "cw_last_error", "cw_stats", "cw_pool_bytes", "cw_pool_offset", "cw_q_roped_offset",
            "cw_order", "cw_predict", "cw_order_arm", "cw_observe", "cw_mark_stale", "cw_feedback", "cw_matched_docs", "cw_feedback_tokens", "cw_hash_chain", "cw_lookup", "cw_release", "cw_extend", "cw_free_list",
            "cw_reset", "cw_admit_batch", "cw_release_batch",
-           "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_prefill_attn_static", "cw_prefill_requests_ws_bytes",
+           "cw_append_kv", "cw_attn_work_ints", "cw_prefill_attn", "cw_attn_schedule", "cw_attn_run", "cw_prefill_attn_static", "cw_prefill_requests_ws_bytes",
            "cw_prefill_requests_work_offset", "cw_prefill_requests", "cw_gather_kv", "cw_prefill_host_ws_bytes",
            "cw_prefill_host"]
 
@@ -330,6 +332,18 @@ class Context:
                                              d_kv_len.data_ptr() if d_kv_len is not None else None, d_tables.data_ptr(),
                                              max_blocks, B, T, int(max_q_len), int(max_kv_len), d_work.data_ptr(),
                                              self._stream()))
+
+    def cw_attn_schedule(self, d_cu, d_nc, d_tables, max_blocks, B, T, max_q_len, max_kv_len, d_work, d_kv_len=None):
+        """first launch of cw_prefill_attn alone: descriptors -> work list (may run before / beside cw_append_kv)."""
+        self._check(self.lib.cw_attn_schedule(self.h, d_cu.data_ptr(), d_nc.data_ptr(),
+                                              d_kv_len.data_ptr() if d_kv_len is not None else None, d_tables.data_ptr(),
+                                              max_blocks, B, T, int(max_q_len), int(max_kv_len), d_work.data_ptr(),
+                                              self._stream()))
+
+    def cw_attn_run(self, q_roped, out, d_tables, max_blocks, B, T, d_work):
+        """second launch of cw_prefill_attn alone: the attention kernel over the list cw_attn_schedule wrote."""
+        self._check(self.lib.cw_attn_run(self.h, q_roped.data_ptr(), out.data_ptr(), d_tables.data_ptr(), max_blocks, B, T,
+                                         d_work.data_ptr(), self._stream()))
 
     def cw_prefill_attn_static(self, q_roped, out, d_cu, d_nc, d_tables, max_blocks, B, T, max_q_len, max_kv_len,
                                d_status=None, d_kv_len=None):

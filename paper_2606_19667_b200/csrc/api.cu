@@ -126,6 +126,9 @@ void cw_destroy(cw_ctx* ctx) {
         if (st.event) cudaEventDestroy(static_cast<cudaEvent_t>(st.event));
         if (st.host) cudaFreeHost(st.host);
     }
+    if (ctx->sched_fork) cudaEventDestroy(static_cast<cudaEvent_t>(ctx->sched_fork));
+    if (ctx->sched_join) cudaEventDestroy(static_cast<cudaEvent_t>(ctx->sched_join));
+    if (ctx->sched_stream) cudaStreamDestroy(static_cast<cudaStream_t>(ctx->sched_stream));
     if (ctx->copy_in_stream) cudaStreamDestroy(static_cast<cudaStream_t>(ctx->copy_in_stream));
     if (ctx->copy_out_stream) cudaStreamDestroy(static_cast<cudaStream_t>(ctx->copy_out_stream));
     delete ctx->tree;
@@ -450,6 +453,32 @@ int cw_prefill_attn(cw_ctx* ctx, const void* q_roped, void* out, const int32_t* 
     return le ? cuda_fail(ctx, le, "cw_prefill_attn") : CW_OK;
 }
 
+// The two launches of cw_prefill_attn one by one (cacheweaver.h): same checks, same kernels.
+int cw_attn_schedule(cw_ctx* ctx, const int32_t* d_cu, const int32_t* d_nc, const int32_t* d_kv_len, const int32_t* d_tables,
+                     int32_t max_blocks, int32_t B, int32_t T, int32_t max_q_len, int32_t max_kv_len, int32_t* d_work,
+                     void* stream) {
+    if (!ctx || ctx->host_only) return fail(ctx, CW_ERR_INVALID, "cw_attn_schedule: host-only context");
+    if (B < 0 || T < 0 || max_blocks <= 0 || max_q_len < 0 || max_kv_len < 0)
+        return fail(ctx, CW_ERR_INVALID, "cw_attn_schedule: bad sizes");
+    if (T == 0 || B == 0) return CW_OK;
+    if (!d_cu || !d_nc || !d_tables || !d_work) return fail(ctx, CW_ERR_INVALID, "cw_attn_schedule: null pointer");
+    if (max_q_len > T || (int64_t)max_kv_len > (int64_t)max_blocks * CW_BLOCK_SIZE || max_kv_len > ctx->cfg.max_position)
+        return fail(ctx, CW_ERR_INVALID, "cw_attn_schedule: max_q_len / max_kv_len exceed T, the block table or max_position");
+    int le = cw::launch_attn_schedule(ctx->cfg, d_cu, d_nc, d_kv_len, d_tables, max_blocks, B, T, max_q_len, max_kv_len,
+                                      d_work, stream);
+    return le ? cuda_fail(ctx, le, "cw_attn_schedule") : CW_OK;
+}
+
+int cw_attn_run(cw_ctx* ctx, const void* q_roped, void* out, const int32_t* d_tables, int32_t max_blocks, int32_t B,
+                int32_t T, int32_t* d_work, void* stream) {
+    if (!ctx || ctx->host_only) return fail(ctx, CW_ERR_INVALID, "cw_attn_run: host-only context");
+    if (B < 0 || T < 0 || max_blocks <= 0) return fail(ctx, CW_ERR_INVALID, "cw_attn_run: bad sizes");
+    if (T == 0 || B == 0) return CW_OK;
+    if (!q_roped || !out || !d_tables || !d_work) return fail(ctx, CW_ERR_INVALID, "cw_attn_run: null pointer");
+    int le = cw::launch_attn_run(ctx->cfg, q_roped, out, d_tables, max_blocks, B, T, d_work, ctx->num_sms, stream);
+    return le ? cuda_fail(ctx, le, "cw_attn_run") : CW_OK;
+}
+
 // cw_prefill_attn with the work list in the library's static device array: for callers that cannot allocate device memory
 // (cacheweaver.h).  Nothing here or below allocates; a batch that needs more than CW_STATIC_WORK_INTS ints is refused.
 int cw_prefill_attn_static(cw_ctx* ctx, const void* q_roped, void* out, const int32_t* d_cu, const int32_t* d_nc,
@@ -475,6 +504,9 @@ int cw_prefill_attn_static(cw_ctx* ctx, const void* q_roped, void* out, const in
 
 // ---- one call per wave: descriptors from the request handles, one staged H2D copy, three launches ----------
 namespace {
+// cw_prefill_requests: waves with at least this many suffix rows run the schedule kernel on a side stream beside
+// cw_append_kv (below it the two event calls cost the host more than the ~20 us the GPU saves)
+constexpr int32_t kSideScheduleMinRows = 4096;
 struct ReqWsLayout {
     int64_t cu, nc, tables, work, total;
 };
@@ -560,10 +592,42 @@ int cw_prefill_requests(cw_ctx* ctx, const int64_t* reqs, int32_t B, const void*
     const int32_t* d_cu = reinterpret_cast<const int32_t*>(ws + w.cu);
     const int32_t* d_nc = reinterpret_cast<const int32_t*>(ws + w.nc);
     const int32_t* d_tables = reinterpret_cast<const int32_t*>(ws + w.tables);
-    int rc = cw_append_kv(ctx, q, k, v, q_roped, d_cu, d_nc, d_tables, max_blocks, B, T, stream);
-    if (rc != CW_OK) return rc;
-    rc = cw_prefill_attn(ctx, q_roped, out, d_cu, d_nc, nullptr, d_tables, max_blocks, B, T, max_q, max_kv,
-                         reinterpret_cast<int32_t*>(ws + w.work), stream);
+    int32_t* d_work = reinterpret_cast<int32_t*>(ws + w.work);
+    int rc;
+    if (T >= kSideScheduleMinRows) {
+        // The schedule kernel needs only the descriptors: it runs on a side stream BESIDE cw_append_kv (one CTA next to an
+        // HBM-bound kernel) instead of between it and the attention kernel.  fork: behind the descriptor copy (and behind
+        // everything earlier on `stream`, so the previous call's attention kernel is done with a shared d_ws); join: in
+        // front of the attention kernel.
+        if (!ctx->sched_stream) {
+            cudaStream_t ss;
+            cudaEvent_t ef, ej;
+            if ((e = cudaStreamCreateWithFlags(&ss, cudaStreamNonBlocking)) != cudaSuccess ||
+                (e = cudaEventCreateWithFlags(&ef, cudaEventDisableTiming)) != cudaSuccess ||
+                (e = cudaEventCreateWithFlags(&ej, cudaEventDisableTiming)) != cudaSuccess)
+                return cuda_fail(ctx, (int)e, "cw_prefill_requests (side stream)");
+            ctx->sched_stream = ss;
+            ctx->sched_fork = ef;
+            ctx->sched_join = ej;
+        }
+        auto ss = static_cast<cudaStream_t>(ctx->sched_stream);
+        auto ef = static_cast<cudaEvent_t>(ctx->sched_fork), ej = static_cast<cudaEvent_t>(ctx->sched_join);
+        if ((e = cudaEventRecord(ef, s)) != cudaSuccess || (e = cudaStreamWaitEvent(ss, ef, 0)) != cudaSuccess)
+            return cuda_fail(ctx, (int)e, "cw_prefill_requests (fork)");
+        rc = cw_attn_schedule(ctx, d_cu, d_nc, nullptr, d_tables, max_blocks, B, T, max_q, max_kv, d_work, ss);
+        // the join is enqueued whatever happened in between: the side stream must never be left un-joined
+        e = cudaEventRecord(ej, ss);
+        const int rc2 = cw_append_kv(ctx, q, k, v, q_roped, d_cu, d_nc, d_tables, max_blocks, B, T, stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s, ej, 0);
+        if (rc != CW_OK) return rc;
+        if (rc2 != CW_OK) return rc2;
+        if (e != cudaSuccess) return cuda_fail(ctx, (int)e, "cw_prefill_requests (join)");
+        rc = cw_attn_run(ctx, q_roped, out, d_tables, max_blocks, B, T, d_work, stream);
+    } else {
+        rc = cw_append_kv(ctx, q, k, v, q_roped, d_cu, d_nc, d_tables, max_blocks, B, T, stream);
+        if (rc != CW_OK) return rc;
+        rc = cw_prefill_attn(ctx, q_roped, out, d_cu, d_nc, nullptr, d_tables, max_blocks, B, T, max_q, max_kv, d_work, stream);
+    }
     if (rc != CW_OK) return rc;
     // Only now, with the copy and both kernels enqueued, do the handles move on: everything up to n is (being) written and
     // the next call starts there.  After a failure above they are unchanged, so the same call can be repeated (writing a

@@ -156,6 +156,10 @@ struct cw_ctx {
         size_t cap = 0;
         void* event = nullptr;
     };
+    // cw_prefill_requests: side stream the schedule kernel runs on beside cw_append_kv, and its fork / join events
+    void* sched_stream = nullptr;
+    void* sched_fork = nullptr;
+    void* sched_join = nullptr;
     static constexpr int kStagingSlots = 4;
     Staging staging[kStagingSlots];
     int staging_next = 0;
@@ -174,6 +178,12 @@ int64_t attn_work_ints(const cw_config& cfg, int32_t B, int32_t T);
 int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* d_cu, const int32_t* d_nc,
                         const int32_t* d_kv_len, const int32_t* tables, int32_t max_blocks, int32_t B, int32_t T,
                         int32_t max_q_len, int32_t max_kv_len, int32_t* d_work, int num_sms, void* stream);
+// its two launches separately: descriptors -> item list (needs no q_roped / KV), then the attention kernel over that list
+int launch_attn_schedule(const cw_config& cfg, const int32_t* d_cu, const int32_t* d_nc, const int32_t* d_kv_len,
+                         const int32_t* tables, int32_t max_blocks, int32_t B, int32_t T, int32_t max_q_len,
+                         int32_t max_kv_len, int32_t* d_work, void* stream);
+int launch_attn_run(const cw_config& cfg, const void* q_roped, void* out, const int32_t* tables, int32_t max_blocks,
+                    int32_t B, int32_t T, int32_t* d_work, int num_sms, void* stream);
 // the same with the work list in the library's own static device array (no caller scratch; at most CW_STATIC_WORK_INTS ints);
 // d_status (device int32[4], may be null) receives the work header
 int launch_prefill_attn_static(const cw_config& cfg, const void* q_roped, void* out, const int32_t* d_cu,

@@ -782,16 +782,33 @@ int64_t attn_work_ints(const cw_config& cfg, int32_t B, int32_t T) {
     return kWorkInts * (attn_max_items(cfg, B, T) + 1);   // + header
 }
 
+// The two launches of cw_prefill_attn can be enqueued apart: the schedule kernel needs only the descriptors, so a caller
+// may run it in front of (or, on another stream, beside) cw_append_kv and keep it off the append -> attention chain.
+int launch_attn_schedule(const cw_config& cfg, const int32_t* d_cu, const int32_t* d_nc, const int32_t* d_kv_len,
+                         const int32_t* tables, int32_t max_blocks, int32_t B, int32_t T, int32_t max_q_len,
+                         int32_t max_kv_len, int32_t* d_work, void* stream) {
+    const int64_t max_items = attn_max_items(cfg, B, T);
+    if (max_items == 0) return 0;
+    attn_schedule_kernel<<<1, 1024, 0, static_cast<cudaStream_t>(stream)>>>(
+        d_cu, d_nc, d_kv_len, tables, cfg.num_blocks, B, T, cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim, max_blocks,
+        cfg.max_position, max_q_len, max_kv_len, d_work, max_items);
+    return (int)cudaGetLastError();
+}
+
 int launch_prefill_attn(const cw_config& cfg, const void* q_roped, void* out, const int32_t* d_cu, const int32_t* d_nc,
                         const int32_t* d_kv_len, const int32_t* tables, int32_t max_blocks, int32_t B, int32_t T,
                         int32_t max_q_len, int32_t max_kv_len, int32_t* d_work, int num_sms, void* stream) {
+    const int le = launch_attn_schedule(cfg, d_cu, d_nc, d_kv_len, tables, max_blocks, B, T, max_q_len, max_kv_len, d_work,
+                                        stream);
+    return le ? le : launch_attn_run(cfg, q_roped, out, tables, max_blocks, B, T, d_work, num_sms, stream);
+}
+
+int launch_attn_run(const cw_config& cfg, const void* q_roped, void* out, const int32_t* tables, int32_t max_blocks,
+                    int32_t B, int32_t T, int32_t* d_work, int num_sms, void* stream) {
     auto s = static_cast<cudaStream_t>(stream);
     const int64_t max_items = attn_max_items(cfg, B, T);
     if (max_items == 0) return 0;
-    attn_schedule_kernel<<<1, 1024, 0, s>>>(d_cu, d_nc, d_kv_len, tables, cfg.num_blocks, B, T, cfg.num_q_heads, cfg.num_kv_heads, cfg.head_dim,
-                                            max_blocks, cfg.max_position, max_q_len, max_kv_len, d_work, max_items);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return (int)e;
+    cudaError_t e = cudaSuccess;
     const float scale_log2 = 1.4426950408889634f / sqrtf((float)cfg.head_dim);
     const unsigned grid = (unsigned)std::min<int64_t>(max_items, num_sms);
     // The dynamic shared memory opt-in is a per-device attribute of the kernel: one flag per device ordinal (a process may

@@ -608,3 +608,27 @@ def test_append_kv_skips_rows_of_a_non_monotone_cu(dev):
     torch.cuda.synchronize()
     assert torch.all(buf[:guard] == 7.0) and torch.all(buf[guard + T * Hq * D:] == 7.0), "store outside q_roped"
     assert torch.isfinite(buf.float()).all()
+
+
+def test_schedule_in_front_of_append_equals_one_call(dev):
+    """cw_attn_schedule needs only the descriptors: enqueued BEFORE cw_append_kv (the pools still hold nothing of the suffix)
+    and followed by cw_attn_run, it gives bit for bit what cw_prefill_attn gives, and the same work header."""
+    b = Batch(dev, 32, 8, 128, cs=[0, 48, 16, 128], ss=[300, 77, 1, 200], seed=21)
+    _, out_ref, cu = b.run()
+    hdr_ref = b.work_header.copy()
+    b2 = Batch(dev, 32, 8, 128, cs=[0, 48, 16, 128], ss=[300, 77, 1, 200], seed=21)
+    b2._append([0] * b2.B, b2.cs)
+    cu2 = np.zeros(b2.B + 1, dtype=np.int32)
+    cu2[1:] = np.cumsum(b2.ss)
+    T = int(cu2[-1])
+    d_cu = torch.from_numpy(cu2).to(dev)
+    d_nc = torch.from_numpy(np.asarray(b2.cs, dtype=np.int32)).to(dev)
+    d_work = torch.empty(b2.ctx.cw_attn_work_ints(b2.B, T), dtype=torch.int32, device=dev)
+    b2.ctx.cw_attn_schedule(d_cu, d_nc, b2.d_tables, b2.max_blocks, b2.B, T, max(b2.ss), max(b2.ns), d_work)
+    qr, *_ = b2._append(b2.cs, b2.ns)
+    out = torch.full_like(qr, float("nan"))
+    b2.ctx.cw_attn_run(qr, out, b2.d_tables, b2.max_blocks, b2.B, T, d_work)
+    torch.cuda.synchronize()
+    assert np.array_equal(to_bits(out), out_ref)
+    hdr = d_work[:8].cpu().numpy()
+    assert hdr[1] == 0 and hdr[3] == hdr_ref[3]
