@@ -407,6 +407,31 @@ def timed(torch, fn, steps, dist):
     return ms
 
 
+def measure_record(torch, wl, pk, local, warmup, seconds=0.0, steps=0):
+    """Attention and append figures of one workload over `steps` steps (or about `seconds` of steps), with the clocks sampled
+    inside that very region: device time by CUDA events, fractions against the burst and the sustained measured peaks."""
+    cfg = wl.cfg
+    with ClockSampler(local) as clk:
+        for _ in range(warmup):
+            wl.step()
+        if seconds > 0:      # device time of a few steps -> number of steps that fill `seconds`
+            ms0 = timed(torch, wl.step, 3, None) / 3
+            steps = max(steps, int(np.ceil(1.25 * seconds * 1e3 / max(1e-3, ms0))))   # 3 cold steps overstate the steady-state step
+        ev = []
+        clk.begin()
+        ms = timed(torch, lambda: wl.step(ev), steps, None) / steps
+        clk.end()
+    app_ms = sum(e[0].elapsed_time(e[1]) for e in ev) / steps
+    attn_ms = sum(e[1].elapsed_time(e[2]) for e in ev) / steps
+    attn_tflops = wl.flops / (attn_ms * 1e-3) / 1e12
+    app_gbs = append_bytes(cfg, wl.T) / (app_ms * 1e-3) / 1e9
+    return {"workload": cfg.name, "requests": cfg.n_req, "waves": len(wl.waves), "steps": steps, "ms_per_step": ms,
+            "seconds": ms * steps * 1e-3, "suffix_tokens": wl.T, "hit_blocks": wl.hit_blocks,
+            "attn_ms": attn_ms, "attn_tflops": attn_tflops, "attn_frac": attn_tflops / pk["bf16"],
+            "attn_frac_of_sustained": attn_tflops / pk["bf16_sustained"],
+            "append_ms": app_ms, "append_gbs": app_gbs, "append_frac": app_gbs / pk["hbm"], "clocks": clk.summary()}
+
+
 def run_ours(args):
     import torch
     rank, local, world = dist_env()
@@ -459,6 +484,12 @@ def run_ours(args):
         ms_e2e = timed(torch, wl.step_e2e, e2e_steps, dist) / e2e_steps
         e2e_value = aggregate_value(wl.flops, ms_e2e, world)
 
+    # the sustained figure (the same step for >= 2 s: clocks settle under the power cap) beside the burst one
+    sustained = None
+    if world == 1 and args.sustained_seconds > 0 and args.seconds <= 0:
+        sustained = measure_record(torch, wl, pk, local, 0, seconds=args.sustained_seconds)
+        sustained["what"] = f"the step of this line repeated for ~{args.sustained_seconds:g} s"
+
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -497,6 +528,23 @@ def run_ours(args):
 
     if cfg.name.startswith("cfg1"):
         prefill["arms_cfg1"] = cfg1_four_arms(device)
+    # the HBM target of cw_append_kv is judged on the concurrent configs 4 and 5 (waves with eviction); their
+    # figures ride along on the default line (timing-only activations drawn on the device; parity at these shapes:
+    # tests/test_gpu_full_size.py)
+    other = None
+    if world == 1 and args.config == 2 and not args.skip_configs and not args.device_inputs:
+        other = {}
+        if hasattr(wl, "host_inputs"):
+            del wl.host_inputs, wl.ws
+        wl.inputs = None
+        torch.cuda.empty_cache()
+        for cid in (4, 5):
+            wo = Workload(cid, args.arm, device, want_e2e=False, device_inputs=True, real_waves=0)
+            rec = measure_record(torch, wo, pk, local, 3, seconds=args.configs_seconds)
+            rec["inputs"] = "device-drawn N(0,1) activations (timing only)"
+            other[f"cfg{cid}"] = rec
+            del wo
+            torch.cuda.empty_cache()
     cpu = None
     if world == 1 or rank == 0:
         sample = OracleSample(cfg_sel, args.oracle_requests, args.oracle_rows)
@@ -529,6 +577,8 @@ def run_ours(args):
                          "window": "attention kernel (cw_attn_run), CUDA events on the launching stream; the schedule kernel runs on a side stream beside cw_append_kv, inside the append window",
                          "peak_source": pk["source"], "frac_of_sustained": attn_tflops / pk["bf16_sustained"],
                          "flops_per_step": wl.flops, "avg_ms": attn_ms / n_l, "launches_per_step": n_l},
+            "sustained": sustained,
+            "configs": other,
             "roofline_append_kv": {"kernel": "append_kv_kernel", "bound": "hbm", "achieved": app_gbs, "peak": pk["hbm"],
                                    "unit": "GB/s", "frac": app_gbs / pk["hbm"], "traffic": traffic_from_profile(cfg.name, "append_kv_kernel"),
                                    "bytes_per_step": append_bytes(cfg, wl.T), "avg_ms": app_ms / n_l},
@@ -781,6 +831,9 @@ def main():
     ap.add_argument("--real-waves", type=int, default=0, help="with --device-inputs: tracegen activations for the first N waves")
     ap.add_argument("--seconds", type=float, default=0.0, help="run the timed region for about this long (sustained figure)")
     ap.add_argument("--skip-per-request", action="store_true")
+    ap.add_argument("--sustained-seconds", type=float, default=2.0, help="length of the extra sustained-clocks record (0 = none)")
+    ap.add_argument("--skip-configs", action="store_true", help="no configs.cfg4 / configs.cfg5 records on the default line")
+    ap.add_argument("--configs-seconds", type=float, default=1.0, help="timed length of each configs.* record")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--oracle-requests", type=int, default=None, help="requests in the oracle's bounded sample")
     ap.add_argument("--oracle-rows", type=int, default=None, help="suffix rows per request in the oracle's bounded sample")

@@ -65,17 +65,25 @@ __global__ void __launch_bounds__(THREADS) append_kv_kernel(
     const int g = Hq / Hkv, tpt = 128 / g;
     const int uq = Hq * CPH, uk = Hkv * CPH;
     const int units = uq + 2 * uk;
+    // A CTA's tokens ascend, so most of them belong to the request of the token before: its descriptor is kept in registers
+    // and the binary search (a chain of dependent loads in front of every token's payload loads) only runs when a token
+    // leaves [q_begin, q_end).
+    int r = -1, q_begin = 0, q_end = 0, nc_r = 0;
     for (int tok = blockIdx.x; tok < T; tok += gridDim.x) {
-        // request of this token: largest r with cu[r] <= tok
-        int lo = 0, hi = B;
-        while (hi - lo > 1) {
-            int mid = (lo + hi) >> 1;
-            if (__ldg(cu + mid) <= tok) lo = mid; else hi = mid;
+        if (r < 0 || tok < q_begin || tok >= q_end) {
+            // request of this token: largest r with cu[r] <= tok
+            int lo = 0, hi = B;
+            while (hi - lo > 1) {
+                int mid = (lo + hi) >> 1;
+                if (__ldg(cu + mid) <= tok) lo = mid; else hi = mid;
+            }
+            r = lo;
+            q_begin = __ldg(cu + r);
+            q_end = __ldg(cu + r + 1);
+            nc_r = __ldg(ncached + r);
         }
-        const int r = lo;
-        const int q_begin = __ldg(cu + r);
-        const int s_len = __ldg(cu + r + 1) - q_begin, tl = tok - q_begin;
-        int p = __ldg(ncached + r) + tl;
+        const int s_len = q_end - q_begin, tl = tok - q_begin;
+        int p = nc_r + tl;
         // q_roped tile: tpt tokens x g heads per (kv head, tile); rows of a tile are stored [64-dim half][row][64], 128B-swizzled
         const int qt = tl / tpt, tloc = tl - qt * tpt;
         const int rows_valid = min(tpt, s_len - qt * tpt) * g;
