@@ -731,6 +731,51 @@ def run_mixed(args):
         del q, k, v, qr, out
 
 
+def run_length_sweep(args):
+    """Item-length sweep of the attention kernel (short items pay the per-item cost): B cold prompts of L tokens
+    each, B * L = 65 536 suffix rows in every case, 8B head shape, attention kernel only (cw_attn_run over a prepared item
+    list), device-drawn activations.  One JSON line per length: ms, TFLOP/s over algorithmic flops, fraction of the peak."""
+    import torch
+    from paper_2606_19667_b200 import Context
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device; there is no CPU fallback")
+    dev, pk = "cuda:0", peaks()
+    Hq, Hkv, D, rows = 32, 8, 128, 65536
+    g = torch.Generator(device=dev)
+    g.manual_seed(0)
+    for L in (64, 128, 256, 512, 1024, 2048, 4096, 8192):
+        B = rows // L
+        mb = L // 16
+        ctx = Context(B * mb + 8, Hq, Hkv, D, 4, rope_theta=5e5, max_position=L, device=dev)
+        tables = torch.arange(B * mb, dtype=torch.int32, device=dev).reshape(B, mb).contiguous()
+        d_cu = torch.arange(0, rows + 1, L, dtype=torch.int32, device=dev)
+        d_nc = torch.zeros(B, dtype=torch.int32, device=dev)
+        q = torch.randn(rows, Hq, D, device=dev, dtype=torch.bfloat16, generator=g)
+        k = torch.randn(rows, Hkv, D, device=dev, dtype=torch.bfloat16, generator=g)
+        v = torch.randn(rows, Hkv, D, device=dev, dtype=torch.bfloat16, generator=g)
+        qr, out = torch.empty_like(q), torch.empty_like(q)
+        work = torch.empty(ctx.cw_attn_work_ints(B, rows), dtype=torch.int32, device=dev)
+        ctx.cw_append_kv(q, k, v, qr, d_cu, d_nc, tables, mb, B, rows)
+
+        def fn():      # the schedule kernel resets the claim counter; only the attention kernel is inside the events
+            ctx.cw_attn_schedule(d_cu, d_nc, tables, mb, B, rows, L, L, work)
+        ms = 0.0
+        for i in range(max(3, args.warmup) + args.steps):
+            fn()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.cw_attn_run(qr, out, tables, mb, B, rows, work)
+            e1.record()
+            torch.cuda.synchronize()
+            if i >= max(3, args.warmup):
+                ms += e0.elapsed_time(e1) / args.steps
+        flops = B * 4 * Hq * D * (L * (L + 1) // 2)
+        print(json.dumps({"prompt_tokens": L, "requests": B, "rows": rows, "items": int(work[3]), "attn_ms": ms,
+                          "attn_tflops": flops / ms / 1e9, "frac_of_bf16_peak": flops / ms / 1e9 / pk["bf16"],
+                          "us_per_item": 1e3 * ms * 148 / max(1, int(work[3]))}), flush=True)
+        del q, k, v, qr, out, ctx
+
+
 def run_layouts(args):
     """config 2's trace under the paper-literal prompt layout (instruction + [Document r: id] headers,
     180-220-token documents) against the block-aligned plain layout with the same retrieval lists:
@@ -842,6 +887,7 @@ def main():
     ap.add_argument("--device-inputs", action="store_true", help="timing-only: draw q,k,v on the device (no e2e leg)")
     ap.add_argument("--layouts", action="store_true", help="NEXT-3: paper-literal prompt layout vs the aligned plain layout, one JSON line per layout and arm")
     ap.add_argument("--mixed", action="store_true", help="NEXT-4: decode rows / prefill suffixes / both in one varlen launch, one JSON line each")
+    ap.add_argument("--length-sweep", action="store_true", help="attention kernel alone on cold prompts of 64..8192 tokens (65 536 rows each), one JSON line per length")
     ap.add_argument("--arms", action="store_true", help="ordering arms of the paper's Table 4 on --config, one JSON line per arm")
     ap.add_argument("--sweep", action="store_true", help="overlap x top-k sweep (BASELINE.json configs[2]), one JSON line per cell")
     args = ap.parse_args()
@@ -850,7 +896,9 @@ def main():
         args.oracle_requests = {1: 4, 2: 16 if args.impl == "ours" else 4, 3: 4, 4: 1, 5: 1}[args.config]
     if args.oracle_rows is None and args.config == 5:
         args.oracle_rows = 4096           # ~12 s instead of ~70 s for the whole 10 304-token prompt
-    if args.layouts:
+    if args.length_sweep:
+        run_length_sweep(args)
+    elif args.layouts:
         run_layouts(args)
     elif args.mixed:
         run_mixed(args)
