@@ -407,6 +407,18 @@ def timed(torch, fn, steps, dist):
     return ms
 
 
+def prefill_saved(cfg, waves):
+    """Per-request share of the prefill that the prefix cache saved (Table 13 reports this per
+    request): token-weighted n_cached / n and flops-weighted c(c+1) / n(n+1) (causal attention pairs), p50 / mean / p95 over
+    the requests of the trace.  Statistics of the admission's answers; nothing of the method is computed here."""
+    c = np.concatenate([np.asarray(w.nc, dtype=np.float64) for w in waves])
+    n = float(cfg.n)
+    out = {}
+    for name, x in (("token_weighted", c / n), ("flops_weighted", c * (c + 1) / (n * (n + 1)))):
+        out[name] = {"p50": float(np.percentile(x, 50)), "mean": float(x.mean()), "p95": float(np.percentile(x, 95))}
+    return out
+
+
 def measure_record(torch, wl, pk, local, warmup, seconds=0.0, steps=0):
     """Attention and append figures of one workload over `steps` steps (or about `seconds` of steps), with the clocks sampled
     inside that very region: device time by CUDA events, fractions against the burst and the sustained measured peaks."""
@@ -499,7 +511,8 @@ def run_ours(args):
     prefill = {args.arm: {"ms": app_ms + attn_ms, "append_ms": app_ms, "attn_ms": attn_ms, "suffix_tokens": wl.T,
                           "hit_blocks": wl.hit_blocks, "attn_flops": wl.flops, "waves": len(wl.waves),
                           "predicted_prefix_docs": pred["predicted_prefix_docs"], "actual_prefix_docs": pred["actual_prefix_docs"],
-                          "over_predicted_docs": pred["over_predicted_docs"], "stale_marks": pred["stale_marks"]}}
+                          "over_predicted_docs": pred["over_predicted_docs"], "stale_marks": pred["stale_marks"],
+                          "prefill_saved": prefill_saved(cfg, wl.waves)}}
     if not args.skip_retrieval:
         del wl.host_inputs, wl.ws
         wr = Workload(cfg_sel, "retrieval", device, want_e2e=False, device_inputs=args.device_inputs, real_waves=args.real_waves)
@@ -510,7 +523,8 @@ def run_ours(args):
         r_app = sum(e[0].elapsed_time(e[1]) for e in ev) / args.steps
         r_attn = sum(e[1].elapsed_time(e[2]) for e in ev) / args.steps
         prefill["retrieval"] = {"ms": r_app + r_attn, "append_ms": r_app, "attn_ms": r_attn, "suffix_tokens": wr.T,
-                                "hit_blocks": wr.hit_blocks, "attn_flops": wr.flops, "waves": len(wr.waves)}
+                                "hit_blocks": wr.hit_blocks, "attn_flops": wr.flops, "waves": len(wr.waves),
+                                "prefill_saved": prefill_saved(cfg, wr.waves)}
         prefill["ratio_measured"] = prefill[args.arm]["ms"] / prefill["retrieval"]["ms"]
         prefill["ratio_predicted_by_flops"] = wl.flops / wr.flops
         del wr
@@ -563,7 +577,9 @@ def run_ours(args):
                        "order": args.arm, "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "inputs": ("tracegen activations (keyed by document prefix)" if not args.device_inputs else
                                   f"tracegen activations for the first {min(args.real_waves, n_l)} wave(s), device-drawn N(0,1) for the rest"),
-                       "l2": "inputs larger than L2 (q,k,v,pool >> 126 MB per step); no explicit flush"},
+                       "l2": "inputs larger than L2 (q,k,v,pool >> 126 MB per step); no explicit flush",
+                       "adjacent_jaccard_mean": float(np.mean([tracegen.jaccard(a, b) for a, b in
+                                                               zip(wl.trace.retrieval[:-1], wl.trace.retrieval[1:])]))},
             "pct_of_bf16_peak": 100.0 * value / world / pk["bf16"],
             "clocks": clk.summary(),
             "e2e": ({"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": wl.h2d // e2e_steps,
